@@ -1,0 +1,168 @@
+/*
+ * swiglu_oracle.c -- CPU oracle for the gated-MLP hot path.  TEST INFRASTRUCTURE ONLY.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may call this.  It shares no code, header, table or helper with the CUDA path under
+ * paper_2607_02521_b200/csrc/, and neither side includes the other.
+ *
+ * What it computes (section 3.1, Eq. 1-3):
+ *
+ *     Gate = A x W1            (Eq. 1)      A  in R^{M x K}
+ *     Up   = A x W2            (Eq. 2)      W1, W2 in R^{K x N}
+ *     Y    = SiLU(Gate) (.) Up (Eq. 3)      SiLU(x) = x * sigma(x)      (line 94)
+ *
+ * The method is exact ("produce the same output (Y) as the unfused
+ * baseline"), so the oracle is the plain definition written out, in fp64, from the same
+ * bf16 input bits the GPU sees (BASELINE.json north_star: "accumulates in fp64 from the
+ * same bf16 inputs").  The result is NOT rounded to bf16: y_ref stays in fp64 and the
+ * tolerance |y - y_ref| <= 2e-3 + 1.6e-2*|y_ref| is applied by the caller.
+ *
+ * Loop structure: outputs are independent, so they are handed out to threads as
+ * (row m, panel of <= PANEL consecutive columns n).  Inside one unit every output's two
+ * dot products are summed with k ascending, exactly as Eq. 1-2 are written; no split of
+ * the k sum, no reassociation, no fused multiply-add is requested (-ffp-contract=off is
+ * passed by the build), no -ffast-math.  Each product of two bf16 values has at most a
+ * 16-bit significand and is exact in fp64; only the k-sum rounds (<= K * 2^-53 relative
+ * to sum |terms|).
+ *
+ * Pins (tests/test_oracle_pins.py): brute-force Fraction arithmetic on tiny shapes; the
+ * hand-worked 2x2x2 example in tests/golden/; SiLU closed forms from 50-digit decimal
+ * arithmetic; SiLU(x)-SiLU(-x)=x reducing Y to two library fp64 matmuls; A=0 => Y=0;
+ * W2=W1 => Y=G*SiLU(G) >= 0; exact scaling / permutation / prefix properties.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define PANEL 256 /* columns per work unit: partition of independent outputs, not of any sum */
+
+/* bf16 -> fp64, exact: a bf16 is the upper 16 bits of an IEEE-754 binary32. */
+static inline double bf16_bits_to_f64(uint16_t h) {
+  uint32_t w = ((uint32_t)h) << 16;
+  float f;
+  memcpy(&f, &w, sizeof f);
+  return (double)f;
+}
+
+/* SiLU(x) = x * sigma(x) = x / (1 + exp(-x))   (line 169 gives the same
+ * form x * (1 + exp(-x))^-1).  For x < 0 the algebraically identical x*e^x/(1+e^x) is used
+ * so exp never overflows (reading R3): finite x gives a finite result. */
+double swiglu_oracle_silu(double x) {
+  if (x >= 0.0) {
+    return x / (1.0 + exp(-x));
+  } else {
+    double e = exp(x);
+    return x * e / (1.0 + e);
+  }
+}
+
+/* One work unit: row m, columns [n0, n1).  gate/up are caller-provided scratch of PANEL. */
+static void unit(const uint16_t *A, const uint16_t *W1, const uint16_t *W2, double *Y,
+                 int64_t N, int64_t K, int64_t m, int64_t n0, int64_t n1, double *gate,
+                 double *up) {
+  const int64_t w = n1 - n0;
+  for (int64_t j = 0; j < w; ++j) {
+    gate[j] = 0.0;
+    up[j] = 0.0;
+  }
+  for (int64_t k = 0; k < K; ++k) { /* k ascending: the sums of Eq. 1 and Eq. 2 */
+    const double a = bf16_bits_to_f64(A[m * K + k]);
+    const uint16_t *w1 = W1 + k * N + n0; /* W[k, n], row-major [K, N] */
+    const uint16_t *w2 = W2 + k * N + n0;
+    for (int64_t j = 0; j < w; ++j) {
+      gate[j] += a * bf16_bits_to_f64(w1[j]); /* Eq. 1 */
+      up[j] += a * bf16_bits_to_f64(w2[j]);   /* Eq. 2 */
+    }
+  }
+  for (int64_t j = 0; j < w; ++j) {
+    Y[m * N + n0 + j] = swiglu_oracle_silu(gate[j]) * up[j]; /* Eq. 3 */
+  }
+}
+
+/*
+ * Y[M,N] (fp64, row-major) = SiLU(A.W1) (.) (A.W2), A[M,K], W1/W2[K,N] given as bf16 bit
+ * patterns (uint16), row-major, dense.  nthreads <= 0 means "all OpenMP threads".
+ * Returns the number of threads used, or -1 on bad arguments.
+ */
+int swiglu_oracle(const uint16_t *A, const uint16_t *W1, const uint16_t *W2, double *Y,
+                  int64_t M, int64_t N, int64_t K, int nthreads) {
+  if (M < 0 || N < 0 || K < 0) return -1;
+  if (M == 0 || N == 0) return 0;
+  if (!A && K > 0) return -1;
+  if ((!W1 || !W2) && K > 0) return -1;
+  if (!Y) return -1;
+  const int64_t panels = (N + PANEL - 1) / PANEL;
+  const int64_t units = M * panels;
+  int used = 1;
+#ifdef _OPENMP
+  if (nthreads <= 0) nthreads = omp_get_max_threads();
+  if ((int64_t)nthreads > units) nthreads = (int)units;
+  used = nthreads;
+#pragma omp parallel num_threads(nthreads)
+#endif
+  {
+    double gate[PANEL], up[PANEL];
+#ifdef _OPENMP
+#pragma omp for schedule(dynamic, 1)
+#endif
+    for (int64_t u = 0; u < units; ++u) {
+      /* panel-major so that threads working at the same time share a W panel in cache */
+      const int64_t p = u / M, m = u % M;
+      const int64_t n0 = p * PANEL;
+      const int64_t n1 = (n0 + PANEL < N) ? n0 + PANEL : N;
+      unit(A, W1, W2, Y, N, K, m, n0, n1, gate, up);
+    }
+  }
+  return used;
+}
+
+/*
+ * Sampled form for full-size shapes: the same computation for a list of `count` rows
+ * (row indices into A) only.  Ysub is [count, N] fp64.  Rows are independent (Eq. 1-3
+ * act row-wise on A), so Ysub[i,:] == Y[rows[i],:] of the full result.
+ */
+int swiglu_oracle_rows(const uint16_t *A, const uint16_t *W1, const uint16_t *W2,
+                       double *Ysub, const int64_t *rows, int64_t count, int64_t M,
+                       int64_t N, int64_t K, int nthreads) {
+  if (M < 0 || N < 0 || K < 0 || count < 0) return -1;
+  if (count == 0 || N == 0) return 0;
+  if (!rows || !Ysub) return -1;
+  if ((!A || !W1 || !W2) && K > 0) return -1;
+  for (int64_t i = 0; i < count; ++i)
+    if (rows[i] < 0 || rows[i] >= M) return -1;
+  const int64_t panels = (N + PANEL - 1) / PANEL;
+  const int64_t units = count * panels;
+  int used = 1;
+#ifdef _OPENMP
+  if (nthreads <= 0) nthreads = omp_get_max_threads();
+  if ((int64_t)nthreads > units) nthreads = (int)units;
+  used = nthreads;
+#pragma omp parallel num_threads(nthreads)
+#endif
+  {
+    double gate[PANEL], up[PANEL];
+#ifdef _OPENMP
+#pragma omp for schedule(dynamic, 1)
+#endif
+    for (int64_t u = 0; u < units; ++u) {
+      const int64_t p = u / count, i = u % count;
+      const int64_t n0 = p * PANEL;
+      const int64_t n1 = (n0 + PANEL < N) ? n0 + PANEL : N;
+      /* write row i of Ysub from row rows[i] of A: shift the base pointers accordingly */
+      unit(A + rows[i] * K, W1, W2, Ysub + i * N, N, K, 0, n0, n1, gate, up);
+    }
+  }
+  return used;
+}
+
+int swiglu_oracle_max_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
