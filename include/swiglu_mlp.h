@@ -1,0 +1,130 @@
+/*
+ * swiglu_mlp.h -- C ABI of libswiglu_b200.so: the fused gated MLP of arxiv/paper_2607_02521
+ * ("Tile-Level Activation Overlap for Efficient LLM Inference") for NVIDIA B200 (sm_100a).
+ *
+ * Operation (section 3.1, Eq. 1-3; problem statement line 74:
+ * "accept the same input tensors (A, W1, W2) and produce the same output (Y) as the
+ * unfused baseline"):
+ *
+ *     Gate = A . W1,   Up = A . W2,   Y = SiLU(Gate) (.) Up,   SiLU(x) = x * sigma(x)
+ *
+ * Numeric contract ("BF16 precision throughout", line 370 "FP32
+ * arithmetic on register-resident values ... BF16 conversion only at the final store"):
+ * bf16 inputs, fp32 accumulation over all of K on the tensor cores, SiLU and the product in
+ * fp32, ONE round-to-nearest-even conversion to bf16 at the store.  In the fused entry
+ * point Gate and Up never exist in HBM.
+ *
+ * Layout: everything dense row-major, no strides.
+ *     A  : M x K bf16, K contiguous         (device pointer, 16-byte aligned)
+ *     W1 : K x N bf16, N contiguous         (device pointer, 16-byte aligned)
+ *     W2 : K x N bf16, N contiguous         (device pointer, 16-byte aligned)
+ *     Y  : M x N bf16, N contiguous         (device pointer, 16-byte aligned, written)
+ * K and N must be multiples of 8 (16-byte row pitch, a TMA requirement); M is arbitrary.
+ *
+ * All pointers are DEVICE pointers on the current CUDA device unless a parameter says
+ * "host".  `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ * Every compute entry point is asynchronous: it returns after enqueueing on `stream`.
+ *
+ * Ownership: the caller owns A, W1, W2, Y and any workspace and keeps them valid until the
+ * enqueued work has completed.  The 8-argument forms may use a library-owned, lazily grown,
+ * per-device workspace; growing it allocates (never while the stream is capturing -- use
+ * the _ex forms with a caller workspace under CUDA-graph capture).
+ *
+ * Errors: a swiglu_status return code; the library never throws, aborts, prints or
+ * synchronises.  Argument validation happens before any CUDA call, so the validation
+ * codes (1-5) can be exercised on a host without a GPU.  M == 0 is SWIGLU_OK and launches
+ * nothing.  There is NO CPU fallback: without an sm_100 device the compute entry points
+ * return SWIGLU_ERR_ARCH or SWIGLU_ERR_CUDA.
+ *
+ * Determinism: same inputs + same variant => bitwise identical Y (split-K partial sums
+ * are combined in a fixed order).  Thread safety: entry points may be called concurrently
+ * from several host threads.
+ */
+#ifndef SWIGLU_MLP_H_
+#define SWIGLU_MLP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  SWIGLU_OK = 0,
+  SWIGLU_ERR_NULL_POINTER = 1, /* A, W1, W2 or Y is NULL while M > 0                    */
+  SWIGLU_ERR_BAD_SHAPE = 2,    /* M < 0, N <= 0, K <= 0, or a byte count overflows int64 */
+  SWIGLU_ERR_UNSUPPORTED = 3,  /* K % 8 != 0 or N % 8 != 0; or an unknown variant id     */
+  SWIGLU_ERR_MISALIGNED = 4,   /* a base pointer is not 16-byte aligned                  */
+  SWIGLU_ERR_ALIASING = 5,     /* Y overlaps A, W1 or W2                                 */
+  SWIGLU_ERR_ARCH = 6,         /* current device is not compute capability 10.x          */
+  SWIGLU_ERR_WORKSPACE = 7,    /* _ex: workspace NULL / misaligned / too small           */
+  SWIGLU_ERR_CUDA = 8          /* a CUDA runtime/driver call failed: swiglu_last_error() */
+} swiglu_status;
+
+/*
+ * Fused path (Eq. 1-3; the paper's Kernel-1/Kernel-2 idea, lines 124-169, rebuilt
+ * for sm_100a): Y = bf16(SiLU(A.W1) * (A.W2)), Gate/Up held only in tensor memory.
+ * The kernel variant is picked per (M, N, K) from a measured table.
+ */
+int swiglu_mlp(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
+               int64_t K, void* stream);
+
+/*
+ * Unfused comparison path (two GEMMs that write Gate and Up
+ * to HBM as bf16, then an elementwise SiLU-multiply kernel).  Built from this library's own
+ * tcgen05 GEMM and elementwise kernels, no cuBLAS.  Needs 2*M*N*2 bytes of workspace
+ * (library-owned in this form).
+ */
+int swiglu_mlp_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                       int64_t N, int64_t K, void* stream);
+
+/*
+ * Explicit-workspace / forced-variant forms.
+ *   workspace       : device pointer, 256-byte aligned, or NULL if workspace_bytes == 0
+ *   workspace_bytes : size of that buffer; must be >= swiglu_workspace_bytes(...) for the
+ *                     variant that will run
+ *   variant         : -1 = automatic (same choice as the 8-argument form), otherwise an id
+ *                     in [0, swiglu_num_variants(unfused))
+ */
+int swiglu_mlp_ex(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                  int64_t N, int64_t K, void* workspace, size_t workspace_bytes, int variant,
+                  void* stream);
+int swiglu_mlp_unfused_ex(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                          int64_t N, int64_t K, void* workspace, size_t workspace_bytes,
+                          int variant, void* stream);
+
+/* Bytes of workspace the given variant (-1 = automatic) needs; 0 if none or bad arguments.
+ * `unfused` != 0 asks about swiglu_mlp_unfused. */
+size_t swiglu_workspace_bytes(int64_t M, int64_t N, int64_t K, int unfused, int variant);
+
+/* Variant table (fused: unfused == 0).  Names are static strings; NULL for a bad id. */
+int swiglu_num_variants(int unfused);
+const char* swiglu_variant_name(int unfused, int variant);
+/* The variant `-1` resolves to for this shape (host-only table lookup, no CUDA call). */
+int swiglu_selected_variant(int64_t M, int64_t N, int64_t K, int unfused);
+
+/* Number of kernel launches one call with this shape/variant enqueues (for accounting). */
+int swiglu_launches_per_call(int64_t M, int64_t N, int64_t K, int unfused, int variant);
+
+/* Validation only (codes 0-5), no CUDA call: what the compute entry points check first. */
+int swiglu_validate(const void* A, const void* W1, const void* W2, const void* Y, int64_t M,
+                    int64_t N, int64_t K);
+
+/*
+ * Host-buffer convenience form: A, W1, W2, Y are HOST pointers (pageable or pinned).  Copies
+ * the inputs to the device, runs swiglu_mlp (unfused == 0) or swiglu_mlp_unfused, copies Y
+ * back and synchronises `stream` before returning.  Device scratch is library-owned.
+ */
+int swiglu_mlp_host(const void* A_host, const void* W1_host, const void* W2_host,
+                    void* Y_host, int64_t M, int64_t N, int64_t K, int unfused, void* stream);
+
+/* Message for the calling thread's most recent non-OK return; static/thread-local storage. */
+const char* swiglu_last_error(void);
+const char* swiglu_status_string(int status);
+const char* swiglu_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SWIGLU_MLP_H_ */

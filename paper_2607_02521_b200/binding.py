@@ -1,0 +1,201 @@
+"""Thin ctypes binding over libswiglu_b200.so -- same names as include/swiglu_mlp.h.
+
+Argument marshalling only: every step of the computation runs in the library's CUDA
+kernels.  Tensors may be torch CUDA tensors (bf16, contiguous) or raw integer device
+pointers together with explicit M, N, K.  There is no fallback of any kind: if the library
+has not been built, loading raises; if there is no sm_100 device, the calls raise
+SwigluError with the library's status code.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libswiglu_b200.so")
+
+SWIGLU_OK = 0
+SWIGLU_ERR_NULL_POINTER = 1
+SWIGLU_ERR_BAD_SHAPE = 2
+SWIGLU_ERR_UNSUPPORTED = 3
+SWIGLU_ERR_MISALIGNED = 4
+SWIGLU_ERR_ALIASING = 5
+SWIGLU_ERR_ARCH = 6
+SWIGLU_ERR_WORKSPACE = 7
+SWIGLU_ERR_CUDA = 8
+
+EXPORTS = (
+    "swiglu_mlp", "swiglu_mlp_unfused", "swiglu_mlp_ex", "swiglu_mlp_unfused_ex",
+    "swiglu_workspace_bytes", "swiglu_num_variants", "swiglu_variant_name",
+    "swiglu_selected_variant", "swiglu_launches_per_call", "swiglu_validate",
+    "swiglu_mlp_host", "swiglu_last_error", "swiglu_status_string", "swiglu_version",
+)
+
+
+class SwigluError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{status_string(status)} ({status}): {message}")
+        self.status = status
+
+
+_lib = None
+
+
+def load():
+    """Load the C-ABI library.  Raises (loudly) if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2607_02521_b200.build` "
+            "(or __graft_entry__.build()); there is no CPU or PyTorch fallback")
+    lib = ctypes.CDLL(LIB_PATH)
+    p, i64, sz, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_size_t, ctypes.c_int
+    for name in ("swiglu_mlp", "swiglu_mlp_unfused"):
+        f = getattr(lib, name)
+        f.argtypes, f.restype = [p, p, p, p, i64, i64, i64, p], ci
+    for name in ("swiglu_mlp_ex", "swiglu_mlp_unfused_ex"):
+        f = getattr(lib, name)
+        f.argtypes, f.restype = [p, p, p, p, i64, i64, i64, p, sz, ci, p], ci
+    lib.swiglu_workspace_bytes.argtypes, lib.swiglu_workspace_bytes.restype = [i64, i64, i64, ci, ci], sz
+    lib.swiglu_num_variants.argtypes, lib.swiglu_num_variants.restype = [ci], ci
+    lib.swiglu_variant_name.argtypes, lib.swiglu_variant_name.restype = [ci, ci], ctypes.c_char_p
+    lib.swiglu_selected_variant.argtypes, lib.swiglu_selected_variant.restype = [i64, i64, i64, ci], ci
+    lib.swiglu_launches_per_call.argtypes, lib.swiglu_launches_per_call.restype = [i64, i64, i64, ci, ci], ci
+    lib.swiglu_validate.argtypes, lib.swiglu_validate.restype = [p, p, p, p, i64, i64, i64], ci
+    lib.swiglu_mlp_host.argtypes, lib.swiglu_mlp_host.restype = [p, p, p, p, i64, i64, i64, ci, p], ci
+    lib.swiglu_last_error.argtypes, lib.swiglu_last_error.restype = [], ctypes.c_char_p
+    lib.swiglu_status_string.argtypes, lib.swiglu_status_string.restype = [ci], ctypes.c_char_p
+    lib.swiglu_version.argtypes, lib.swiglu_version.restype = [], ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+# ------------------------------------------------------------------ marshalling helpers
+def _ptr(x):
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):      # torch.Tensor
+        return int(x.data_ptr())
+    if hasattr(x, "ctypes"):        # numpy array (host buffers of swiglu_mlp_host)
+        return int(x.ctypes.data)
+    raise TypeError(f"cannot take a pointer from {type(x)}")
+
+
+def _stream(stream):
+    if stream is None:
+        try:
+            import torch
+            if torch.cuda.is_available():
+                return int(torch.cuda.current_stream().cuda_stream)
+        except ImportError:
+            pass
+        return None
+    if isinstance(stream, int):
+        return stream or None
+    return int(stream.cuda_stream)
+
+
+def _dims(A, W1, W2, Y, M, N, K):
+    if M is not None and N is not None and K is not None:
+        return int(M), int(N), int(K)
+    for t, name in ((A, "A"), (W1, "W1"), (W2, "W2"), (Y, "Y")):
+        if not hasattr(t, "shape") or len(t.shape) != 2:
+            raise TypeError(f"{name}: need a 2-D tensor, or pass M, N, K with raw pointers")
+        if hasattr(t, "is_contiguous") and not t.is_contiguous():
+            raise ValueError(f"{name} must be contiguous (dense row-major, no strides)")
+        if hasattr(t, "element_size") and t.element_size() != 2:
+            raise TypeError(f"{name} must hold 2-byte bf16 elements")
+    m, k = A.shape
+    k2, n = W1.shape
+    if k2 != k or tuple(W2.shape) != (k, n) or tuple(Y.shape) != (m, n):
+        raise ValueError(f"shape mismatch: A{tuple(A.shape)} W1{tuple(W1.shape)} "
+                         f"W2{tuple(W2.shape)} Y{tuple(Y.shape)}")
+    return int(m), int(n), int(k)
+
+
+def _check(status: int):
+    if status != SWIGLU_OK:
+        raise SwigluError(status, last_error())
+
+
+# ------------------------------------------------------------------ the ABI, name for name
+def swiglu_mlp(A, W1, W2, Y, M=None, N=None, K=None, stream=None) -> None:
+    """Fused Y = bf16(SiLU(A.W1) * (A.W2)); asynchronous on `stream`."""
+    m, n, k = _dims(A, W1, W2, Y, M, N, K)
+    _check(load().swiglu_mlp(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), m, n, k, _stream(stream)))
+
+
+def swiglu_mlp_unfused(A, W1, W2, Y, M=None, N=None, K=None, stream=None) -> None:
+    """Unfused comparison path: two GEMMs writing bf16 Gate/Up, then SiLU-multiply."""
+    m, n, k = _dims(A, W1, W2, Y, M, N, K)
+    _check(load().swiglu_mlp_unfused(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), m, n, k,
+                                     _stream(stream)))
+
+
+def swiglu_mlp_ex(A, W1, W2, Y, M=None, N=None, K=None, workspace=None, workspace_bytes=0,
+                  variant=-1, stream=None) -> None:
+    m, n, k = _dims(A, W1, W2, Y, M, N, K)
+    _check(load().swiglu_mlp_ex(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), m, n, k, _ptr(workspace),
+                                int(workspace_bytes), int(variant), _stream(stream)))
+
+
+def swiglu_mlp_unfused_ex(A, W1, W2, Y, M=None, N=None, K=None, workspace=None,
+                          workspace_bytes=0, variant=-1, stream=None) -> None:
+    m, n, k = _dims(A, W1, W2, Y, M, N, K)
+    _check(load().swiglu_mlp_unfused_ex(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), m, n, k,
+                                        _ptr(workspace), int(workspace_bytes), int(variant),
+                                        _stream(stream)))
+
+
+def swiglu_mlp_host(A_host, W1_host, W2_host, Y_host, M, N, K, unfused=False, stream=None) -> None:
+    """Host-buffer form: H2D copies, the kernel(s), D2H copy and a stream sync, all inside."""
+    _check(load().swiglu_mlp_host(_ptr(A_host), _ptr(W1_host), _ptr(W2_host), _ptr(Y_host),
+                                  int(M), int(N), int(K), int(bool(unfused)), _stream(stream)))
+
+
+def swiglu_validate(A, W1, W2, Y, M, N, K) -> int:
+    """Returns the status code (no exception): the argument checks, without any CUDA call."""
+    return int(load().swiglu_validate(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), int(M), int(N), int(K)))
+
+
+def swiglu_workspace_bytes(M, N, K, unfused=False, variant=-1) -> int:
+    return int(load().swiglu_workspace_bytes(int(M), int(N), int(K), int(bool(unfused)), int(variant)))
+
+
+def swiglu_num_variants(unfused=False) -> int:
+    return int(load().swiglu_num_variants(int(bool(unfused))))
+
+
+def swiglu_variant_name(variant, unfused=False):
+    s = load().swiglu_variant_name(int(bool(unfused)), int(variant))
+    return None if s is None else s.decode()
+
+
+def swiglu_selected_variant(M, N, K, unfused=False) -> int:
+    return int(load().swiglu_selected_variant(int(M), int(N), int(K), int(bool(unfused))))
+
+
+def swiglu_launches_per_call(M, N, K, unfused=False, variant=-1) -> int:
+    return int(load().swiglu_launches_per_call(int(M), int(N), int(K), int(bool(unfused)), int(variant)))
+
+
+def last_error() -> str:
+    return load().swiglu_last_error().decode()
+
+
+swiglu_last_error = last_error
+
+
+def status_string(status: int) -> str:
+    return load().swiglu_status_string(int(status)).decode()
+
+
+swiglu_status_string = status_string
+
+
+def swiglu_version() -> str:
+    return load().swiglu_version().decode()

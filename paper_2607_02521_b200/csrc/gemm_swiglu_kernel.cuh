@@ -1,0 +1,315 @@
+// gemm_swiglu_kernel.cuh -- the large-M kernel: persistent, warp-specialised, TMA ->
+// smem ring -> tcgen05.mma -> TMEM (double-buffered) -> epilogue -> TMA store.
+//
+// kFused = true : Y[m, n] = bf16( SiLU(A.W1)[m,n] * (A.W2)[m,n] )      (Eq. 1-3)
+//   One UMMA of N = 256 per k-step covers the W1 tile (TMEM columns [0,128) = Gate) and the
+//   W2 tile (columns [128,256) = Up) of the same 128 output columns: the tile-level form of
+//   the paper's Kernel-2 "[M,2N]" pairing with no interleaved
+//   weight copy, and of Kernel-1's "both accumulators in one threadblock" (lines 130-139)
+//   with A streamed once instead of twice.  SiLU-multiply of tile i runs in the epilogue
+//   warps while the MMA warp accumulates tile i+1 into the other TMEM stage -- the sm_100
+//   counterpart of the paper's Swish-under-loads / SwiGLU-under-stores overlaps (lines 128,
+//   165).
+// kFused = false: C[m, n] = bf16( (A.W)[m,n] ), a plain GEMM with 256-column tiles; used
+//   twice (Gate, Up) by the unfused comparison path.
+//
+// kCtaGroup = 1: one CTA per 128-row tile.  kCtaGroup = 2: a CTA pair (cluster 2x1) shares one
+//   256-row tile; each CTA loads its 128 rows of A and HALF of the B columns (fused: rank 0
+//   loads the W1 tile, rank 1 the W2 tile), the leader issues cta_group::2 MMAs.
+#pragma once
+#include <cuda.h>
+
+#include "sm100_ptx.cuh"
+
+namespace swiglu {
+
+using namespace sm100;
+
+constexpr int BM = 128;      // rows of A / Y per CTA
+constexpr int BK = 64;       // k per pipeline stage: 64 bf16 = one 128-byte swizzle row
+constexpr int UMMA_K = 16;   // k per tcgen05.mma (kind::f16)
+constexpr int UMMA_N = 256;  // accumulator columns per tile
+constexpr int kEpiWarps = 4;
+constexpr int kGemmThreads = 64 + 32 * kEpiWarps;  // warp 0 TMA, warp 1 MMA, warps 2-5 epilogue
+constexpr int kTmemCols = 512;                     // 2 accumulator stages x 256 columns
+constexpr int kOutBufBytes = BM * 64 * 2;          // one 64-column bf16 output chunk (16 KB)
+
+template <int kCtaGroup>
+struct GemmCfg {
+  static constexpr int kBColsPerCta = UMMA_N / kCtaGroup;
+  static constexpr int kABytes = BM * BK * 2;            // 16 KB
+  static constexpr int kBBytes = kBColsPerCta * BK * 2;  // 32 KB (1-CTA) / 16 KB (2-CTA)
+  static constexpr int kStageBytes = kABytes + kBBytes;
+  static constexpr int kStages = (kCtaGroup == 1) ? 4 : 6;
+  static constexpr int kBarBytes = 1024;
+  // +1024: slack to align the dynamic smem base to 1024 B (128-byte swizzle atoms)
+  static constexpr int kSmemBytes = kStages * kStageBytes + 2 * kOutBufBytes + kBarBytes + 1024;
+};
+
+struct GemmParams {
+  int M, N, K;
+  int m_tiles;   // ceil(M / (128*kCtaGroup))
+  int n_tiles;   // ceil(N / (fused ? 128 : 256))
+  int group_m;   // m-tiles per L2 raster group
+};
+
+// Tile order: groups of `group_m` row-tiles x all column-tiles, row-tile fastest inside a
+// group, so the CTAs running at one time share a slab of A that stays in L2 and stream W.
+__device__ __forceinline__ void decode_tile(const GemmParams& p, int t, int& tm, int& tn) {
+  const int per_group = p.group_m * p.n_tiles;
+  const int g = t / per_group;
+  const int r = t - g * per_group;
+  const int m0 = g * p.group_m;
+  const int gm = min(p.group_m, p.m_tiles - m0);
+  tn = r / gm;
+  tm = m0 + (r - tn * gm);
+}
+
+__device__ __forceinline__ float silu_mul(float g, float u) {
+  // SiLU(g)*u = g*u / (1 + 2^(-g*log2 e)); fp32 throughout.
+  float e, r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(g * -1.4426950408889634f));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
+  return (g * u) * r;
+}
+
+template <int kCtaGroup, bool kFused>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
+                   const __grid_constant__ CUtensorMap tmap_b1,
+                   const __grid_constant__ CUtensorMap tmap_b2,
+                   const __grid_constant__ CUtensorMap tmap_y, const GemmParams p) {
+  using Cfg = GemmCfg<kCtaGroup>;
+  constexpr int kStages = Cfg::kStages;
+  constexpr int kOutCols = kFused ? 128 : 256;  // output columns per tile
+  constexpr int kChunks = kOutCols / 64;        // 64-column epilogue chunks per tile
+
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t smem_out = smem_base + kStages * Cfg::kStageBytes;
+  const uint32_t bar_base = smem_out + 2 * kOutBufBytes;
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (kStages + s); };
+  auto acc_full_bar = [&](int a) { return bar_base + 8u * (2 * kStages + a); };
+  auto acc_empty_bar = [&](int a) { return bar_base + 8u * (2 * kStages + 2 + a); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * kStages + 4);
+  auto smem_a = [&](int s) { return smem_base + s * Cfg::kStageBytes; };
+  auto smem_b = [&](int s) { return smem_base + s * Cfg::kStageBytes + Cfg::kABytes; };
+
+  const uint32_t warp = threadIdx.x >> 5;
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t rank = (kCtaGroup == 2) ? cluster_ctarank() : 0u;
+  const int num_groups = gridDim.x / kCtaGroup;  // CTAs (or CTA pairs) sharing the tile list
+  const int group_id = blockIdx.x / kCtaGroup;
+  const int total_tiles = p.m_tiles * p.n_tiles;
+  const int k_blocks = (p.K + BK - 1) / BK;
+
+  // ------------------------------------------------------------------ one-time setup
+  if (warp == 0 && lane == 0) {
+    prefetch_tensormap(&tmap_a);
+    prefetch_tensormap(&tmap_b1);
+    if (kFused) prefetch_tensormap(&tmap_b2);
+    prefetch_tensormap(&tmap_y);
+    for (int s = 0; s < kStages; ++s) {
+      mbar_init(full_bar(s), 1);
+      mbar_init(empty_bar(s), 1);
+    }
+    for (int a = 0; a < 2; ++a) {
+      mbar_init(acc_full_bar(a), 1);
+      mbar_init(acc_empty_bar(a), kEpiWarps * kCtaGroup);
+    }
+    fence_mbar_init();
+  }
+  if (warp == 1) tmem_alloc<kCtaGroup>(tmem_slot, kTmemCols);
+  tcgen05_fence_before();
+  if (kCtaGroup == 2) cluster_sync(); else __syncthreads();
+  tcgen05_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  // PDL: everything above overlapped the previous kernel's tail; its output (and, for the
+  // unfused path, the Gate/Up it wrote) must be complete before we touch global memory.
+  pdl_wait_prior_grid();
+  pdl_launch_dependents();  // the next kernel may start its own prologue as SMs free up
+
+  if (warp == 0 && lane == 0) {
+    // ================================================================ TMA producer
+    int s = 0;
+    uint32_t ph = 0;
+    for (int t = group_id; t < total_tiles; t += num_groups) {
+      int tm, tn;
+      decode_tile(p, t, tm, tn);
+      const int m_base = (tm * kCtaGroup + (int)rank) * BM;
+      const int n_base = tn * kOutCols;
+      for (int kb = 0; kb < k_blocks; ++kb) {
+        mbar_wait(empty_bar(s), ph ^ 1u);
+        if (rank == 0) mbar_arrive_expect_tx(full_bar(s), Cfg::kStageBytes * kCtaGroup);
+        const int k0 = kb * BK;
+        const uint32_t sa = smem_a(s), sb = smem_b(s), fb = full_bar(s);
+        if constexpr (kCtaGroup == 1) {
+          tma_load_2d(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
+          if constexpr (kFused) {
+            tma_load_2d(sb, &tmap_b1, fb, n_base, k0, kEvictNormal);
+            tma_load_2d(sb + 8192, &tmap_b1, fb, n_base + 64, k0, kEvictNormal);
+            tma_load_2d(sb + 16384, &tmap_b2, fb, n_base, k0, kEvictNormal);
+            tma_load_2d(sb + 24576, &tmap_b2, fb, n_base + 64, k0, kEvictNormal);
+          } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+              tma_load_2d(sb + j * 8192, &tmap_b1, fb, n_base + j * 64, k0, kEvictNormal);
+          }
+        } else {
+          tma_load_2d_pair(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
+          if constexpr (kFused) {
+            const CUtensorMap* tb = (rank == 0) ? &tmap_b1 : &tmap_b2;
+            tma_load_2d_pair(sb, tb, fb, n_base, k0, kEvictNormal);
+            tma_load_2d_pair(sb + 8192, tb, fb, n_base + 64, k0, kEvictNormal);
+          } else {
+            const int nb = n_base + (int)rank * 128;
+            tma_load_2d_pair(sb, &tmap_b1, fb, nb, k0, kEvictNormal);
+            tma_load_2d_pair(sb + 8192, &tmap_b1, fb, nb + 64, k0, kEvictNormal);
+          }
+        }
+        if (++s == kStages) { s = 0; ph ^= 1u; }
+      }
+    }
+  } else if (warp == 1 && lane == 0 && rank == 0) {
+    // ================================================================ MMA issuer
+    constexpr uint32_t idesc = idesc_bf16_f32(BM * kCtaGroup, UMMA_N, /*a_mn=*/false,
+                                              /*b_mn=*/true);
+    int s = 0;
+    uint32_t ph = 0;
+    int it = 0;
+    for (int t = group_id; t < total_tiles; t += num_groups, ++it) {
+      const int as = it & 1;
+      const uint32_t aph = (it >> 1) & 1u;
+      mbar_wait(acc_empty_bar(as), aph ^ 1u);  // epilogue has drained this TMEM stage
+      tcgen05_fence_after();
+      const uint32_t d_tmem = tmem_base + as * UMMA_N;
+      for (int kb = 0; kb < k_blocks; ++kb) {
+        mbar_wait(full_bar(s), ph);
+        tcgen05_fence_after();
+        const uint32_t sa = smem_a(s), sb = smem_b(s);
+#pragma unroll
+        for (int k = 0; k < BK / UMMA_K; ++k) {
+          // A: K-major, +32 B per 16-k step inside the 128-byte swizzle row.
+          const uint64_t adesc = smem_desc_sw128(sa + k * (UMMA_K * 2), 16, 1024);
+          // B: MN-major, 16 k rows = 2 KB per step; 64-column atoms 8 KB apart.
+          const uint64_t bdesc = smem_desc_sw128(sb + k * (UMMA_K * 128), 8192, 1024);
+          umma_bf16<kCtaGroup>(d_tmem, adesc, bdesc, idesc, (kb | k) != 0 ? 1u : 0u);
+        }
+        umma_commit<kCtaGroup>(empty_bar(s));  // smem stage free once these MMAs retire
+        if (++s == kStages) { s = 0; ph ^= 1u; }
+      }
+      umma_commit<kCtaGroup>(acc_full_bar(as));  // accumulator complete -> epilogue
+    }
+  } else if (warp >= 2) {
+    // ================================================================ epilogue
+    const uint32_t q = warp & 3u;  // TMEM lane quarter this warp may read
+    const uint32_t row = q * 32u + lane;
+    const bool issuer = (threadIdx.x == 64);
+    const uint32_t leader_acc_empty0 = (kCtaGroup == 2) ? mapa_shared(acc_empty_bar(0), 0) : 0u;
+    int it = 0;
+    uint32_t chunk_ctr = 0;
+    for (int t = group_id; t < total_tiles; t += num_groups, ++it) {
+      int tm, tn;
+      decode_tile(p, t, tm, tn);
+      const int m_base = (tm * kCtaGroup + (int)rank) * BM;
+      const int n_base = tn * kOutCols;
+      const int as = it & 1;
+      const uint32_t aph = (it >> 1) & 1u;
+      mbar_wait(acc_full_bar(as), aph);
+      tcgen05_fence_after();
+      const uint32_t tacc = tmem_base + ((q * 32u) << 16) + as * UMMA_N;
+#pragma unroll 1
+      for (int h = 0; h < kChunks; ++h, ++chunk_ctr) {
+        const uint32_t obuf = smem_out + (chunk_ctr & 1u) * kOutBufBytes;
+        // the TMA store that last read this buffer (2 chunks ago) must have finished reading
+        if (issuer) tma_store_wait_read<1>();
+        named_bar_sync(1, kEpiWarps * 32);
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+          uint32_t packed[16];
+          if constexpr (kFused) {
+            uint32_t g[32], u[32];
+            tmem_ld_32x32b_x32(tacc + h * 64 + c * 32, g);
+            tmem_ld_32x32b_x32(tacc + 128 + h * 64 + c * 32, u);
+            tmem_ld_wait();
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+              const float y0 = silu_mul(__uint_as_float(g[2 * j]), __uint_as_float(u[2 * j]));
+              const float y1 =
+                  silu_mul(__uint_as_float(g[2 * j + 1]), __uint_as_float(u[2 * j + 1]));
+              packed[j] = pack_bf16x2_rn(y0, y1);
+            }
+          } else {
+            uint32_t v[32];
+            tmem_ld_32x32b_x32(tacc + h * 64 + c * 32, v);
+            tmem_ld_wait();
+#pragma unroll
+            for (int j = 0; j < 16; ++j)
+              packed[j] = pack_bf16x2_rn(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
+          }
+          if (h == kChunks - 1 && c == 1) {
+            // last TMEM read of this tile is done: hand the accumulator stage back to the MMA
+            tcgen05_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+              if constexpr (kCtaGroup == 2) mbar_arrive_cluster(leader_acc_empty0 + 8u * as);
+              else mbar_arrive(acc_empty_bar(as));
+            }
+          }
+          // 128-byte swizzled staging: row r, 16-byte chunk j -> chunk (j ^ (r & 7))
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const uint32_t chunk = (uint32_t)(c * 4 + j) ^ (row & 7u);
+            st_shared_v4(obuf + row * 128u + chunk * 16u, packed[4 * j], packed[4 * j + 1],
+                         packed[4 * j + 2], packed[4 * j + 3]);
+          }
+        }
+        fence_proxy_async_smem();
+        named_bar_sync(1, kEpiWarps * 32);
+        if (issuer) {
+          tma_store_2d(&tmap_y, obuf, n_base + h * 64, m_base);  // OOB rows/cols are clipped
+          tma_store_commit();
+        }
+      }
+    }
+    if (issuer) tma_store_wait_all<0>();
+  }
+
+  // ------------------------------------------------------------------ teardown
+  __syncwarp();
+  tcgen05_fence_before();
+  if (kCtaGroup == 2) cluster_sync(); else __syncthreads();
+  if (warp == 1) {
+    tcgen05_fence_after();
+    tmem_dealloc<kCtaGroup>(tmem_base, kTmemCols);
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// Elementwise stage of the unfused path: Y = bf16( SiLU(float(G)) * float(U) )
+// (read Gate, read Up, write Y).  16-byte vector accesses.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+silu_mul_kernel(const uint4* __restrict__ G, const uint4* __restrict__ U, uint4* __restrict__ Y,
+                int64_t n_vec) {
+  pdl_wait_prior_grid();
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_vec; i += stride) {
+    const uint4 g = __ldg(G + i), u = __ldg(U + i);
+    const uint32_t gw[4] = {g.x, g.y, g.z, g.w}, uw[4] = {u.x, u.y, u.z, u.w};
+    uint32_t yw[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const float g0 = __uint_as_float(gw[j] << 16), g1 = __uint_as_float(gw[j] & 0xFFFF0000u);
+      const float u0 = __uint_as_float(uw[j] << 16), u1 = __uint_as_float(uw[j] & 0xFFFF0000u);
+      yw[j] = pack_bf16x2_rn(silu_mul(g0, u0), silu_mul(g1, u1));
+    }
+    Y[i] = make_uint4(yw[0], yw[1], yw[2], yw[3]);
+  }
+  pdl_launch_dependents();
+}
+
+}  // namespace swiglu

@@ -1,0 +1,537 @@
+// swiglu_api.cu -- the C ABI of include/swiglu_mlp.h: validation, variant table, tensor
+// maps, workspace, launches.  Host logic only; the kernels are in the .cuh files.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include "../../include/swiglu_mlp.h"
+#include "gemm_swiglu_kernel.cuh"
+#include "smallm_swiglu_kernel.cuh"
+
+namespace {
+
+// ------------------------------------------------------------------ error bookkeeping
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof g_err, fmt, ap);
+  va_end(ap);
+  return code;
+}
+int fail_cuda(cudaError_t e, const char* what) {
+  return fail(SWIGLU_ERR_CUDA, "%s: %s (%s)", what, cudaGetErrorName(e), cudaGetErrorString(e));
+}
+#define CUDA_TRY(expr)                                   \
+  do {                                                   \
+    cudaError_t _e = (expr);                             \
+    if (_e != cudaSuccess) return fail_cuda(_e, #expr);  \
+  } while (0)
+
+// ------------------------------------------------------------------ variant tables
+enum FusedVariant {
+  kFused1Cta = 0,     // 128x128 (Gate|Up) tile per CTA
+  kFused2Cta = 1,     // 256x128 tile per CTA pair, cta_group::2
+  kFusedSmallM = 2,   // swap-AB, split-K over a cluster, for M <= 64
+  kNumFused = 3
+};
+enum UnfusedVariant { kUnfused1Cta = 0, kUnfused2Cta = 1, kNumUnfused = 2 };
+const char* const kFusedNames[kNumFused] = {"fused_1cta_128x128", "fused_2cta_256x128",
+                                            "fused_smallm_swapab_splitk"};
+const char* const kUnfusedNames[kNumUnfused] = {"unfused_1cta_gemm128x256+silu_mul",
+                                                "unfused_2cta_gemm256x256+silu_mul"};
+
+int env_int(const char* name, int dflt) {
+  const char* v = getenv(name);
+  return (v && *v) ? atoi(v) : dflt;
+}
+
+// Measured dispatch (table regenerated from bench sweeps).
+int select_fused(int64_t M, int64_t N, int64_t K) {
+  (void)N; (void)K;
+  const int forced = env_int("SWIGLU_VARIANT", -1);
+  if (forced >= 0 && forced < kNumFused) {
+    if (forced != kFusedSmallM || M <= swiglu::kSmallMMax) return forced;
+  }
+  if (M <= swiglu::kSmallMMax) return kFusedSmallM;
+  if (M <= 128) return kFused1Cta;
+  return kFused2Cta;
+}
+int select_unfused(int64_t M, int64_t N, int64_t K) {
+  (void)N; (void)K;
+  const int forced = env_int("SWIGLU_UNFUSED_VARIANT", -1);
+  if (forced >= 0 && forced < kNumUnfused) return forced;
+  return (M <= 128) ? kUnfused1Cta : kUnfused2Cta;
+}
+
+// ------------------------------------------------------------------ validation (no CUDA)
+bool overlaps(const void* a, int64_t abytes, const void* b, int64_t bbytes) {
+  const uintptr_t a0 = (uintptr_t)a, a1 = a0 + (uintptr_t)abytes;
+  const uintptr_t b0 = (uintptr_t)b, b1 = b0 + (uintptr_t)bbytes;
+  return a0 < b1 && b0 < a1;
+}
+bool mul_overflows(int64_t a, int64_t b, int64_t limit) { return a != 0 && b > limit / a; }
+
+int validate(const void* A, const void* W1, const void* W2, const void* Y, int64_t M, int64_t N,
+             int64_t K) {
+  if (M < 0 || N <= 0 || K <= 0)
+    return fail(SWIGLU_ERR_BAD_SHAPE, "bad shape M=%lld N=%lld K=%lld (need M>=0, N>0, K>0)",
+                (long long)M, (long long)N, (long long)K);
+  const int64_t lim = INT64_MAX / 4;
+  if (mul_overflows(M, K, lim) || mul_overflows(K, N, lim) || mul_overflows(M, N, lim) ||
+      M > INT32_MAX - 256 || N > INT32_MAX - 256 || K > INT32_MAX - 256)
+    return fail(SWIGLU_ERR_BAD_SHAPE, "shape too large M=%lld N=%lld K=%lld", (long long)M,
+                (long long)N, (long long)K);
+  if ((K % 8) != 0 || (N % 8) != 0)
+    return fail(SWIGLU_ERR_UNSUPPORTED,
+                "K=%lld and N=%lld must be multiples of 8 (16-byte row pitch for TMA)",
+                (long long)K, (long long)N);
+  if (M == 0) return SWIGLU_OK;
+  if (!A || !W1 || !W2 || !Y) return fail(SWIGLU_ERR_NULL_POINTER, "A, W1, W2 or Y is NULL");
+  if (((uintptr_t)A | (uintptr_t)W1 | (uintptr_t)W2 | (uintptr_t)Y) & 15u)
+    return fail(SWIGLU_ERR_MISALIGNED, "A, W1, W2 and Y must be 16-byte aligned");
+  const int64_t ab = M * K * 2, wb = K * N * 2, yb = M * N * 2;
+  if (overlaps(Y, yb, A, ab) || overlaps(Y, yb, W1, wb) || overlaps(Y, yb, W2, wb))
+    return fail(SWIGLU_ERR_ALIASING, "Y overlaps an input");
+  return SWIGLU_OK;
+}
+
+// ------------------------------------------------------------------ device state
+struct DeviceState {
+  bool ready = false;
+  int device = -1;
+  int sm_count = 0;
+  int cc_major = 0;
+  void* workspace = nullptr;
+  size_t workspace_bytes = 0;
+  void* host_scratch = nullptr;  // device scratch of swiglu_mlp_host
+  size_t host_scratch_bytes = 0;
+};
+std::mutex g_mu;
+DeviceState g_dev[64];
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn g_encode = nullptr;
+
+int get_device_state(DeviceState** out) {
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return fail(SWIGLU_ERR_CUDA, "device index %d out of range", dev);
+  std::lock_guard<std::mutex> lk(g_mu);
+  DeviceState& d = g_dev[dev];
+  if (!d.ready) {
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+    d.device = dev;
+    d.sm_count = prop.multiProcessorCount;
+    d.cc_major = prop.major;
+    if (prop.major != 10)
+      return fail(SWIGLU_ERR_ARCH, "device %d is sm_%d%d; this library is sm_100a only", dev,
+                  prop.major, prop.minor);
+    if (!g_encode) {
+      void* fn = nullptr;
+      cudaDriverEntryPointQueryResult qres;
+      CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+      if (!fn || qres != cudaDriverEntryPointSuccess)
+        return fail(SWIGLU_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
+      g_encode = (EncodeTiledFn)fn;
+    }
+    using namespace swiglu;
+    CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  GemmCfg<1>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, false>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  GemmCfg<1>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, true>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  GemmCfg<2>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, false>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  GemmCfg<2>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  SmallCfg<16>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  SmallCfg<32>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  SmallCfg<64>::kSmemBytes));
+    d.ready = true;
+  }
+  *out = &d;
+  return SWIGLU_OK;
+}
+
+// 2-D bf16 row-major tensor [outer, inner] (inner contiguous), box = box_outer x box_inner,
+// 128-byte swizzle (box_inner must be 64 elements), out-of-bounds reads give zeros.
+int make_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
+              uint32_t box_inner, uint32_t box_outer) {
+  const cuuint64_t dims[2] = {(cuuint64_t)inner, (cuuint64_t)outer};
+  const cuuint64_t strides[1] = {(cuuint64_t)inner * 2};
+  const cuuint32_t box[2] = {box_inner, box_outer};
+  const cuuint32_t elem[2] = {1, 1};
+  const CUresult r =
+      g_encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides,
+               box, elem, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS)
+    return fail(SWIGLU_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d) inner=%lld outer=%lld",
+                (int)r, (long long)inner, (long long)outer);
+  return SWIGLU_OK;
+}
+
+bool pdl_enabled() {
+  static const bool on = env_int("SWIGLU_NO_PDL", 0) == 0;
+  return on;
+}
+
+// ------------------------------------------------------------------ launches
+template <int kCtaGroup, bool kFused>
+int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void* B2, void* Yout,
+                int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
+  using namespace swiglu;
+  CUtensorMap ta, tb1, tb2, ty;
+  int rc;
+  if ((rc = make_tmap(&ta, A, K, M, 64, 128))) return rc;
+  if ((rc = make_tmap(&tb1, B1, N, K, 64, 64))) return rc;
+  if ((rc = make_tmap(&tb2, kFused ? B2 : B1, N, K, 64, 64))) return rc;
+  if ((rc = make_tmap(&ty, Yout, N, M, 64, 128))) return rc;
+  GemmParams p;
+  p.M = (int)M; p.N = (int)N; p.K = (int)K;
+  const int rows_per_tile = BM * kCtaGroup;
+  const int out_cols = kFused ? 128 : 256;
+  p.m_tiles = (int)((M + rows_per_tile - 1) / rows_per_tile);
+  p.n_tiles = (int)((N + out_cols - 1) / out_cols);
+  // L2 raster group: keep the slab of A the running CTAs share at <= 32 MiB
+  int64_t gm = (32ll << 20) / ((int64_t)rows_per_tile * K * 2);
+  const int forced_gm = env_int("SWIGLU_GROUP_M", 0);
+  if (forced_gm > 0) gm = forced_gm;
+  if (gm < 1) gm = 1;
+  if (gm > p.m_tiles) gm = p.m_tiles;
+  p.group_m = (int)gm;
+  const int64_t tiles = (int64_t)p.m_tiles * p.n_tiles;
+  int groups = d.sm_count / kCtaGroup;
+  if (tiles < groups) groups = (int)tiles;
+
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof cfg);
+  cfg.gridDim = dim3((unsigned)(groups * kCtaGroup));
+  cfg.blockDim = dim3(kGemmThreads);
+  cfg.dynamicSmemBytes = GemmCfg<kCtaGroup>::kSmemBytes;
+  cfg.stream = stream;
+  cudaLaunchAttribute attrs[2];
+  int na = 0;
+  if (kCtaGroup == 2) {
+    attrs[na].id = cudaLaunchAttributeClusterDimension;
+    attrs[na].val.clusterDim.x = 2;
+    attrs[na].val.clusterDim.y = 1;
+    attrs[na].val.clusterDim.z = 1;
+    ++na;
+  }
+  if (pdl_enabled()) {
+    attrs[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attrs[na].val.programmaticStreamSerializationAllowed = 1;
+    ++na;
+  }
+  cfg.attrs = attrs;
+  cfg.numAttrs = na;
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_swiglu_kernel<kCtaGroup, kFused>, ta, tb1, tb2, ty, p));
+  return SWIGLU_OK;
+}
+
+// Split-K factor of the small-M kernel: as many CTAs as can be co-resident (2 per SM), at
+// most 8 per cluster (portable cluster size), at least one k-block per CTA.
+int smallm_ksplit(int sm_count, int64_t n_tiles, int64_t k_blocks) {
+  const int forced = env_int("SWIGLU_KSPLIT", 0);
+  int64_t s = (2ll * sm_count) / n_tiles;
+  if (forced > 0) s = forced;
+  if (s > 8) s = 8;
+  if (s > k_blocks) s = k_blocks;
+  if (s < 1) s = 1;
+  return (int)s;
+}
+
+template <int MP>
+int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const void* W2,
+                     void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
+  using namespace swiglu;
+  CUtensorMap ta, tw1, tw2;
+  int rc;
+  if ((rc = make_tmap(&ta, A, K, M, 64, MP))) return rc;
+  if ((rc = make_tmap(&tw1, W1, N, K, 64, 64))) return rc;
+  if ((rc = make_tmap(&tw2, W2, N, K, 64, 64))) return rc;
+  const int64_t n_tiles = (N + 127) / 128, k_blocks = (K + BK - 1) / BK;
+  SmallParams p;
+  p.M = (int)M; p.N = (int)N; p.K = (int)K;
+  p.ksplit = smallm_ksplit(d.sm_count, n_tiles, k_blocks);
+  p.ldy = N;
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof cfg);
+  cfg.gridDim = dim3((unsigned)(n_tiles * p.ksplit));
+  cfg.blockDim = dim3(kSmallThreads);
+  cfg.dynamicSmemBytes = SmallCfg<MP>::kSmemBytes;
+  cfg.stream = stream;
+  cudaLaunchAttribute attrs[2];
+  int na = 0;
+  if (p.ksplit > 1) {
+    attrs[na].id = cudaLaunchAttributeClusterDimension;
+    attrs[na].val.clusterDim.x = (unsigned)p.ksplit;
+    attrs[na].val.clusterDim.y = 1;
+    attrs[na].val.clusterDim.z = 1;
+    ++na;
+  }
+  if (pdl_enabled()) {
+    attrs[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attrs[na].val.programmaticStreamSerializationAllowed = 1;
+    ++na;
+  }
+  cfg.attrs = attrs;
+  cfg.numAttrs = na;
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, smallm_swiglu_kernel<MP>, ta, tw1, tw2, (uint16_t*)Y, p));
+  return SWIGLU_OK;
+}
+
+int launch_smallm(const DeviceState& d, const void* A, const void* W1, const void* W2, void* Y,
+                  int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
+  if (M <= 16) return launch_smallm_mp<16>(d, A, W1, W2, Y, M, N, K, stream);
+  if (M <= 32) return launch_smallm_mp<32>(d, A, W1, W2, Y, M, N, K, stream);
+  return launch_smallm_mp<64>(d, A, W1, W2, Y, M, N, K, stream);
+}
+
+int launch_silu_mul(const DeviceState& d, const void* G, const void* U, void* Y, int64_t elems,
+                    cudaStream_t stream) {
+  const int64_t n_vec = elems / 8;  // N % 8 == 0 so M*N % 8 == 0
+  int64_t blocks = (n_vec + 255) / 256;
+  const int64_t cap = (int64_t)d.sm_count * 8;
+  if (blocks > cap) blocks = cap;
+  if (blocks < 1) blocks = 1;
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof cfg);
+  cfg.gridDim = dim3((unsigned)blocks);
+  cfg.blockDim = dim3(256);
+  cfg.stream = stream;
+  cudaLaunchAttribute attrs[1];
+  int na = 0;
+  if (pdl_enabled()) {
+    attrs[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attrs[na].val.programmaticStreamSerializationAllowed = 1;
+    ++na;
+  }
+  cfg.attrs = attrs;
+  cfg.numAttrs = na;
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, swiglu::silu_mul_kernel, (const uint4*)G, (const uint4*)U,
+                              (uint4*)Y, n_vec));
+  return SWIGLU_OK;
+}
+
+size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+size_t workspace_for(int64_t M, int64_t N, int64_t K, int unfused, int variant) {
+  if (M <= 0 || N <= 0 || K <= 0) return 0;
+  if (unfused) return 2 * round_up((size_t)M * N * 2, 256);  // Gate and Up, bf16
+  if (variant < 0) variant = select_fused(M, N, K);
+  (void)variant;
+  return 0;  // fused variants reduce split-K partials on chip (DSMEM), no global workspace
+}
+
+int ensure_workspace(DeviceState& d, size_t need, cudaStream_t stream, void** out) {
+  std::lock_guard<std::mutex> lk(g_mu);
+  if (need > d.workspace_bytes) {
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    cudaStreamIsCapturing(stream, &cap);
+    if (cap != cudaStreamCaptureStatusNone)
+      return fail(SWIGLU_ERR_WORKSPACE,
+                  "library workspace must grow to %zu bytes but the stream is capturing; "
+                  "use the _ex form with a caller workspace", need);
+    if (d.workspace) {
+      CUDA_TRY(cudaDeviceSynchronize());  // earlier calls may still be using the old buffer
+      CUDA_TRY(cudaFree(d.workspace));
+      d.workspace = nullptr;
+      d.workspace_bytes = 0;
+    }
+    CUDA_TRY(cudaMalloc(&d.workspace, need));
+    d.workspace_bytes = need;
+  }
+  *out = d.workspace;
+  return SWIGLU_OK;
+}
+
+int run_fused(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
+              int64_t K, int variant, cudaStream_t stream) {
+  int rc = validate(A, W1, W2, Y, M, N, K);
+  if (rc) return rc;
+  if (variant < -1 || variant >= kNumFused)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
+  if (variant == kFusedSmallM && M > swiglu::kSmallMMax)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "variant %s handles M <= %d only",
+                kFusedNames[kFusedSmallM], swiglu::kSmallMMax);
+  if (M == 0) return SWIGLU_OK;
+  DeviceState* d;
+  if ((rc = get_device_state(&d))) return rc;
+  if (variant < 0) variant = select_fused(M, N, K);
+  switch (variant) {
+    case kFused1Cta: return launch_gemm<1, true>(*d, A, W1, W2, Y, M, N, K, stream);
+    case kFused2Cta: return launch_gemm<2, true>(*d, A, W1, W2, Y, M, N, K, stream);
+    case kFusedSmallM: return launch_smallm(*d, A, W1, W2, Y, M, N, K, stream);
+  }
+  return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
+}
+
+int run_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
+                int64_t K, void* ws, size_t ws_bytes, bool own_ws, int variant,
+                cudaStream_t stream) {
+  int rc = validate(A, W1, W2, Y, M, N, K);
+  if (rc) return rc;
+  if (variant < -1 || variant >= kNumUnfused)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "unknown unfused variant %d", variant);
+  if (M == 0) return SWIGLU_OK;
+  const size_t need = workspace_for(M, N, K, 1, variant);
+  if (!own_ws) {
+    if (!ws || ws_bytes < need || ((uintptr_t)ws & 255u))
+      return fail(SWIGLU_ERR_WORKSPACE, "workspace needs %zu bytes, 256-byte aligned", need);
+  }
+  DeviceState* d;
+  if ((rc = get_device_state(&d))) return rc;
+  if (own_ws && (rc = ensure_workspace(*d, need, stream, &ws))) return rc;
+  if (variant < 0) variant = select_unfused(M, N, K);
+  void* G = ws;
+  void* U = (char*)ws + need / 2;
+  if (variant == kUnfused1Cta) {
+    if ((rc = launch_gemm<1, false>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
+    if ((rc = launch_gemm<1, false>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
+  } else {
+    if ((rc = launch_gemm<2, false>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
+    if ((rc = launch_gemm<2, false>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
+  }
+  return launch_silu_mul(*d, G, U, Y, M * N, stream);
+}
+
+}  // namespace
+
+// ====================================================================== C ABI
+extern "C" {
+
+int swiglu_validate(const void* A, const void* W1, const void* W2, const void* Y, int64_t M,
+                    int64_t N, int64_t K) {
+  return validate(A, W1, W2, Y, M, N, K);
+}
+
+int swiglu_mlp(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
+               int64_t K, void* stream) {
+  return run_fused(A, W1, W2, Y, M, N, K, -1, (cudaStream_t)stream);
+}
+
+int swiglu_mlp_ex(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
+                  int64_t K, void* workspace, size_t workspace_bytes, int variant,
+                  void* stream) {
+  (void)workspace; (void)workspace_bytes;  // no fused variant needs a global workspace
+  return run_fused(A, W1, W2, Y, M, N, K, variant, (cudaStream_t)stream);
+}
+
+int swiglu_mlp_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                       int64_t N, int64_t K, void* stream) {
+  return run_unfused(A, W1, W2, Y, M, N, K, nullptr, 0, true, -1, (cudaStream_t)stream);
+}
+
+int swiglu_mlp_unfused_ex(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                          int64_t N, int64_t K, void* workspace, size_t workspace_bytes,
+                          int variant, void* stream) {
+  return run_unfused(A, W1, W2, Y, M, N, K, workspace, workspace_bytes, false, variant,
+                     (cudaStream_t)stream);
+}
+
+size_t swiglu_workspace_bytes(int64_t M, int64_t N, int64_t K, int unfused, int variant) {
+  return workspace_for(M, N, K, unfused, variant);
+}
+
+int swiglu_num_variants(int unfused) { return unfused ? (int)kNumUnfused : (int)kNumFused; }
+
+const char* swiglu_variant_name(int unfused, int variant) {
+  if (variant < 0 || variant >= (unfused ? (int)kNumUnfused : (int)kNumFused)) return nullptr;
+  return unfused ? kUnfusedNames[variant] : kFusedNames[variant];
+}
+
+int swiglu_selected_variant(int64_t M, int64_t N, int64_t K, int unfused) {
+  return unfused ? select_unfused(M, N, K) : select_fused(M, N, K);
+}
+
+int swiglu_launches_per_call(int64_t M, int64_t N, int64_t K, int unfused, int variant) {
+  (void)N; (void)K; (void)variant;
+  if (M <= 0) return 0;
+  return unfused ? 3 : 1;
+}
+
+int swiglu_mlp_host(const void* A_host, const void* W1_host, const void* W2_host, void* Y_host,
+                    int64_t M, int64_t N, int64_t K, int unfused, void* stream_v) {
+  cudaStream_t stream = (cudaStream_t)stream_v;
+  // validate shapes/pointers with the host pointers (alignment of host buffers is irrelevant)
+  if (M < 0 || N <= 0 || K <= 0) return validate(nullptr, nullptr, nullptr, nullptr, M, N, K);
+  if ((K % 8) || (N % 8)) return validate(nullptr, nullptr, nullptr, nullptr, M, N, K);
+  if (M == 0) return SWIGLU_OK;
+  if (!A_host || !W1_host || !W2_host || !Y_host)
+    return fail(SWIGLU_ERR_NULL_POINTER, "a host pointer is NULL");
+  DeviceState* d;
+  int rc = get_device_state(&d);
+  if (rc) return rc;
+  const size_t ab = round_up((size_t)M * K * 2, 256), wb = round_up((size_t)K * N * 2, 256),
+               yb = round_up((size_t)M * N * 2, 256);
+  const size_t need = ab + 2 * wb + yb;
+  char* base;
+  {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (need > d->host_scratch_bytes) {
+      if (d->host_scratch) {
+        CUDA_TRY(cudaDeviceSynchronize());
+        CUDA_TRY(cudaFree(d->host_scratch));
+        d->host_scratch = nullptr;
+        d->host_scratch_bytes = 0;
+      }
+      CUDA_TRY(cudaMalloc(&d->host_scratch, need));
+      d->host_scratch_bytes = need;
+    }
+    base = (char*)d->host_scratch;
+  }
+  void *dA = base, *dW1 = base + ab, *dW2 = base + ab + wb, *dY = base + ab + 2 * wb;
+  CUDA_TRY(cudaMemcpyAsync(dA, A_host, (size_t)M * K * 2, cudaMemcpyHostToDevice, stream));
+  CUDA_TRY(cudaMemcpyAsync(dW1, W1_host, (size_t)K * N * 2, cudaMemcpyHostToDevice, stream));
+  CUDA_TRY(cudaMemcpyAsync(dW2, W2_host, (size_t)K * N * 2, cudaMemcpyHostToDevice, stream));
+  rc = unfused ? swiglu_mlp_unfused(dA, dW1, dW2, dY, M, N, K, stream_v)
+               : swiglu_mlp(dA, dW1, dW2, dY, M, N, K, stream_v);
+  if (rc) return rc;
+  CUDA_TRY(cudaMemcpyAsync(Y_host, dY, (size_t)M * N * 2, cudaMemcpyDeviceToHost, stream));
+  CUDA_TRY(cudaStreamSynchronize(stream));
+  return SWIGLU_OK;
+}
+
+const char* swiglu_last_error(void) { return g_err; }
+
+const char* swiglu_status_string(int status) {
+  switch (status) {
+    case SWIGLU_OK: return "SWIGLU_OK";
+    case SWIGLU_ERR_NULL_POINTER: return "SWIGLU_ERR_NULL_POINTER";
+    case SWIGLU_ERR_BAD_SHAPE: return "SWIGLU_ERR_BAD_SHAPE";
+    case SWIGLU_ERR_UNSUPPORTED: return "SWIGLU_ERR_UNSUPPORTED";
+    case SWIGLU_ERR_MISALIGNED: return "SWIGLU_ERR_MISALIGNED";
+    case SWIGLU_ERR_ALIASING: return "SWIGLU_ERR_ALIASING";
+    case SWIGLU_ERR_ARCH: return "SWIGLU_ERR_ARCH";
+    case SWIGLU_ERR_WORKSPACE: return "SWIGLU_ERR_WORKSPACE";
+    case SWIGLU_ERR_CUDA: return "SWIGLU_ERR_CUDA";
+  }
+  return "SWIGLU_ERR_UNKNOWN";
+}
+
+const char* swiglu_version(void) { return "swiglu_b200 0.1.0 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,116 @@
+"""Host logic of the C-ABI boundary, no GPU needed: the library loads, exports every symbol
+include/swiglu_mlp.h declares, and rejects bad arguments before any CUDA call."""
+import os
+import re
+
+import pytest
+
+from paper_2607_02521_b200 import binding as B
+from paper_2607_02521_b200 import build as libbuild
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    libbuild.build()
+    return B.load()
+
+
+def test_every_declared_symbol_is_exported(lib):
+    header = open(os.path.join(ROOT, "include", "swiglu_mlp.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(swiglu_[a-z_]+)\s*\(", header))
+    assert declared == set(B.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_version_status_strings_and_variant_table(lib):
+    assert "sm_100a" in B.swiglu_version()
+    assert B.status_string(0) == "SWIGLU_OK" and B.status_string(5) == "SWIGLU_ERR_ALIASING"
+    nf, nu = B.swiglu_num_variants(False), B.swiglu_num_variants(True)
+    assert nf >= 3 and nu >= 1
+    names = [B.swiglu_variant_name(v) for v in range(nf)]
+    assert len(set(names)) == nf and all(names)
+    assert B.swiglu_variant_name(nf) is None and B.swiglu_variant_name(-1) is None
+    # dispatch is a host-side table: decode sizes go to the swap-AB kernel, large M does not
+    small = B.swiglu_variant_name(B.swiglu_selected_variant(16, 4864, 896))
+    large = B.swiglu_variant_name(B.swiglu_selected_variant(4096, 8960, 1536))
+    assert "smallm" in small and "smallm" not in large
+    assert B.swiglu_launches_per_call(16, 4864, 896) == 1
+    assert B.swiglu_launches_per_call(16, 4864, 896, unfused=True) == 3
+    assert B.swiglu_launches_per_call(0, 4864, 896) == 0
+
+
+def test_workspace_query(lib):
+    assert B.swiglu_workspace_bytes(128, 8960, 1536, unfused=False) == 0
+    need = B.swiglu_workspace_bytes(128, 8960, 1536, unfused=True)
+    assert need >= 2 * 128 * 8960 * 2 and need % 256 == 0
+    assert B.swiglu_workspace_bytes(-1, 8, 8, unfused=True) == 0
+
+
+A, W1, W2, Y = 0x10000000, 0x20000000, 0x30000000, 0x40000000  # fake, aligned, disjoint
+
+
+@pytest.mark.parametrize("args,code", [
+    ((A, W1, W2, Y, 16, 4864, 896), B.SWIGLU_OK),
+    ((None, None, None, None, 0, 4864, 896), B.SWIGLU_OK),               # M == 0: nothing to do
+    ((None, W1, W2, Y, 16, 4864, 896), B.SWIGLU_ERR_NULL_POINTER),
+    ((A, W1, W2, None, 16, 4864, 896), B.SWIGLU_ERR_NULL_POINTER),
+    ((A, W1, W2, Y, -1, 4864, 896), B.SWIGLU_ERR_BAD_SHAPE),
+    ((A, W1, W2, Y, 16, 0, 896), B.SWIGLU_ERR_BAD_SHAPE),
+    ((A, W1, W2, Y, 16, 4864, 0), B.SWIGLU_ERR_BAD_SHAPE),
+    ((A, W1, W2, Y, 2**40, 2**30, 2**30), B.SWIGLU_ERR_BAD_SHAPE),       # byte count overflow
+    ((A, W1, W2, Y, 16, 4860, 896), B.SWIGLU_ERR_UNSUPPORTED),           # N % 8
+    ((A, W1, W2, Y, 16, 4864, 900), B.SWIGLU_ERR_UNSUPPORTED),           # K % 8
+    ((A + 2, W1, W2, Y, 16, 4864, 896), B.SWIGLU_ERR_MISALIGNED),
+    ((A, W1, W2, Y + 8, 16, 4864, 896), B.SWIGLU_ERR_MISALIGNED),
+    ((A, W1, W2, A, 16, 4864, 896), B.SWIGLU_ERR_ALIASING),              # Y == A
+    ((A, W1, W2, W2 + 4864 * 2 * 10, 16, 4864, 896), B.SWIGLU_ERR_ALIASING),  # Y inside W2
+    ((A, W1, W2, A - 16 * 4864 * 2 + 16, 16, 4864, 896), B.SWIGLU_ERR_ALIASING),  # Y tail hits A
+])
+def test_validation_codes(lib, args, code):
+    assert B.swiglu_validate(*args) == code
+    if code != B.SWIGLU_OK:
+        assert B.last_error()
+
+
+def test_compute_entry_points_validate_before_touching_cuda(lib):
+    """Bad arguments come back with their own code even on a host without a GPU."""
+    for fn in (B.swiglu_mlp, B.swiglu_mlp_unfused):
+        with pytest.raises(B.SwigluError) as e:
+            fn(A, W1, W2, Y, M=16, N=4860, K=896, stream=0)
+        assert e.value.status == B.SWIGLU_ERR_UNSUPPORTED
+        fn(A, W1, W2, Y, M=0, N=4864, K=896, stream=0)  # M == 0: OK, launches nothing
+    with pytest.raises(B.SwigluError) as e:
+        B.swiglu_mlp_ex(A, W1, W2, Y, M=16, N=4864, K=896, variant=99, stream=0)
+    assert e.value.status == B.SWIGLU_ERR_UNSUPPORTED
+    with pytest.raises(B.SwigluError) as e:
+        B.swiglu_mlp_unfused_ex(A, W1, W2, Y, M=16, N=4864, K=896, workspace=None,
+                                workspace_bytes=0, stream=0)
+    assert e.value.status == B.SWIGLU_ERR_WORKSPACE
+
+
+def test_no_cpu_fallback_without_a_device(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(B.SwigluError) as e:
+        B.swiglu_mlp(A, W1, W2, Y, M=16, N=4864, K=896, stream=0)
+    assert e.value.status in (B.SWIGLU_ERR_CUDA, B.SWIGLU_ERR_ARCH)
+
+
+def test_product_path_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2607_02521_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in text.replace("the oracle", "").replace("oracle's", "") \
+                    or f in ("inputs.py", "check.py"), f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2607_02521_b200" not in text
+            assert "from paper_2607_02521_b200" not in text
