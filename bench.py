@@ -1,0 +1,530 @@
+#!/usr/bin/env python
+"""bench.py -- fused SwiGLU-MLP TFLOP/s and % of roofline per M on B200 (BASELINE.json metric).
+
+    python bench.py --gpus N --steps K --warmup W [--workload qwen2.5-1.5b] [--impl reference]
+    python bench.py --all            # every BASELINE.json point -> gpurun_out/results.{json,md}
+
+A STEP is one pass of the whole hot path over one batch of synthetic input: for the
+workload's (K, N) the fused entry point `swiglu_mlp` is called once per batch size M of that
+BASELINE.json config (1.5B: M = 1, 16, 128, 1024, 4096), which exercises host dispatch, the
+small-M swap-AB/split-K kernel and the large-M tcgen05 kernels.  `value` = sum(4*M*N*K) over
+the step / device time, inputs resident in HBM; weights rotate through enough copies that
+every call streams them from HBM (cold L2).  See DESIGN.md "Measurement".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fused_swiglu_mlp_tflops"
+UNIT = "TFLOP/s"
+NOMINAL = {"bf16_tflops": 2250.0, "hbm_gbs": 8000.0}
+FALLBACK = {"bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "hbm_gbs": 6650.0}
+L2_BYTES = 126 << 20
+
+
+def flops(M, N, K):
+    return 4.0 * M * N * K                      # BASELINE.json: "TFLOP/s, counted as 4*M*N*K"
+
+
+def algo_bytes(M, N, K):
+    return 2 * K * N * 2 + M * K * 2 + M * N * 2  # BASELINE.json: weights + A + Y, once each
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            d = json.load(open(path))
+            return {"bf16_tflops": float(d["bf16_tflops"]),
+                    "bf16_tflops_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"])),
+                    "hbm_gbs": float(d["hbm_gbs"])}, "measured"
+        except Exception:
+            pass
+    return dict(FALLBACK), "fallback"
+
+
+def roofline_time_s(M, N, K, peak_tflops, hbm_gbs):
+    tc = flops(M, N, K) / (peak_tflops * 1e12)
+    tm = algo_bytes(M, N, K) / (hbm_gbs * 1e9)
+    return max(tc, tm), ("tensor" if tc >= tm else "hbm")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, power, reasons = [], None, [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for l in self.lines:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax = float(f[1]); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        # "under load": samples in the top half of the observed power range
+        load = sm
+        if power and max(power) > 1.5 * min(power):
+            cut = (max(power) + min(power)) / 2
+            load = [c for c, p in zip(sm, power) if p >= cut] or sm
+        return {"sm_mhz": statistics.median(load) if load else None, "sm_max_mhz": smax,
+                "power_w_max": max(power) if power else None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------
+# workload: one (K, N) shape with its batch sizes, resident in HBM, weights rotating
+# ---------------------------------------------------------------------------------------
+class Workload:
+    def __init__(self, name, rank=0, rotate=True):
+        import numpy as np
+        import torch
+        from paper_2607_02521_b200 import inputs
+        table = dict(inputs.SHAPES)
+        table.update(inputs.PAPER_SHAPES)
+        self.name = name
+        self.K, self.N, self.seed, self.Ms = table[name]
+        self.Mmax = max(self.Ms)
+        K, N = self.K, self.N
+        self.W1h, self.W2h = inputs.make_weights(K, N, self.seed)
+        # rank r owns rows [r*Mmax, (r+1)*Mmax) of the shape's activation stream
+        allA = inputs.make_activations((rank + 1) * self.Mmax, K, self.seed)
+        self.Ah = np.ascontiguousarray(allA[rank * self.Mmax:])
+        wbytes = 2 * K * N * 2
+        self.copies = 1 if (not rotate or wbytes >= 2 * L2_BYTES) else -(-2 * L2_BYTES // wbytes) + 1
+        to_dev = lambda b: torch.from_numpy(b.view(np.int16)).cuda().view(torch.bfloat16)
+        self.W1 = [to_dev(self.W1h)]
+        self.W2 = [to_dev(self.W2h)]
+        self.A = [to_dev(self.Ah)]
+        for _ in range(self.copies - 1):
+            self.W1.append(self.W1[0].clone())
+            self.W2.append(self.W2[0].clone())
+            self.A.append(self.A[0].clone())
+        self.Y = torch.empty((self.Mmax, N), dtype=torch.bfloat16, device="cuda")
+        self.counter = 0
+        self.l2_note = (f"cold L2: {self.copies} rotating copies of (A, W1, W2), "
+                        f"{self.copies * wbytes / 2**20:.0f} MiB >= 2x L2" if self.copies > 1 else
+                        f"weights {wbytes / 2**20:.0f} MiB per call exceed 2x L2")
+
+    def call(self, fn, M, stream=None):
+        """One C-ABI call with raw device pointers (fn = lib.swiglu_mlp or lib.swiglu_mlp_unfused)."""
+        import torch
+        c = self.counter % self.copies
+        self.counter += 1
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        rc = fn(self.A[c].data_ptr(), self.W1[c].data_ptr(), self.W2[c].data_ptr(),
+                self.Y.data_ptr(), M, self.N, self.K, stream)
+        if rc != 0:
+            from paper_2607_02521_b200 import binding
+            raise binding.SwigluError(rc, binding.last_error())
+
+    def flops_per_step(self):
+        return sum(flops(M, self.N, self.K) for M in self.Ms)
+
+
+def time_point(wl, fn, M, target_ms=1.5, batches=15):
+    """Median / min microseconds per call.  A batch of back-to-back calls (rotating weight
+    copies) is captured once into a CUDA graph and replayed between two CUDA events, so the
+    figure is what a serving loop replaying a captured decode step sees, free of Python
+    launch gaps; calls >= ~100 us are not launch-bound and give the same number either way."""
+    import torch
+    for _ in range(3):
+        wl.call(fn, M)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(3):
+        wl.call(fn, M)
+    e1.record()
+    torch.cuda.synchronize()
+    est_ms = max(e0.elapsed_time(e1) / 3, 1e-3)
+    per = max(wl.copies, min(100, int(round(target_ms / est_ms))))
+    per = -(-per // wl.copies) * wl.copies  # whole rotations: every replay starts at copy 0
+    wl.counter = 0
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        for _ in range(per):
+            wl.call(fn, M)
+    for _ in range(2):
+        g.replay()
+    torch.cuda.synchronize()
+    samples = []
+    for _ in range(batches):
+        e0.record()
+        g.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        samples.append(e0.elapsed_time(e1) * 1e3 / per)
+    med = statistics.median(samples)
+    cv = (statistics.pstdev(samples) / med) if med > 0 else 0.0
+    return {"us_median": med, "us_min": min(samples), "cv": cv, "calls_per_batch": per,
+            "batches": batches}
+
+
+def check_point(wl, M, max_rows=16):
+    """Mismatch counts of both paths against the CPU oracle on sampled rows (tests/ holds the
+    parity tests proper; this is the count the north_star asks to report beside the timing)."""
+    import numpy as np
+    import torch
+    import oracle
+    from paper_2607_02521_b200 import binding as B, check, inputs
+    rows = inputs.sample_rows(M)
+    if len(rows) > max_rows:
+        idx = np.linspace(0, len(rows) - 1, max_rows).round().astype(int)
+        rows = rows[idx]
+    y_ref, _ = oracle.swiglu_oracle_rows(wl.Ah[:M], wl.W1h, wl.W2h, rows)
+    out = {}
+    sel = torch.from_numpy(rows).cuda()
+    lib = B.load()
+    for key, fn in (("fused", lib.swiglu_mlp), ("unfused", lib.swiglu_mlp_unfused)):
+        wl.Y[:M].fill_(float("nan"))
+        wl.call(fn, M)
+        c = (wl.counter - 1) % wl.copies
+        assert c < wl.copies  # all copies hold the same bits as wl.Ah / wl.W1h / wl.W2h
+        torch.cuda.synchronize()
+        y = wl.Y[:M][sel].view(torch.int16).cpu().numpy().view(np.uint16)
+        rep = check.compare(y, y_ref)
+        out[key] = {"mismatches": rep.mismatches, "checked": rep.checked,
+                    "max_ratio": round(rep.max_ratio, 4), "not_rne_of_ref": rep.not_rne_of_ref}
+    return out
+
+
+def measure_points(wl, peaks, do_check=True, Ms=None):
+    from paper_2607_02521_b200 import binding as B
+    pts = []
+    for M in (Ms or wl.Ms):
+        f = time_point(wl, B.load().swiglu_mlp, M)
+        u = time_point(wl, B.load().swiglu_mlp_unfused, M)
+        t = f["us_median"] * 1e-6
+        fl, by = flops(M, wl.N, wl.K), algo_bytes(M, wl.N, wl.K)
+        t_roof, bound = roofline_time_s(M, wl.N, wl.K, peaks["bf16_tflops"], peaks["hbm_gbs"])
+        t_nom, _ = roofline_time_s(M, wl.N, wl.K, NOMINAL["bf16_tflops"], NOMINAL["hbm_gbs"])
+        t_sus, _ = roofline_time_s(M, wl.N, wl.K, peaks["bf16_tflops_sustained"], peaks["hbm_gbs"])
+        p = {"workload": wl.name, "M": M, "N": wl.N, "K": wl.K,
+             "variant": B.swiglu_variant_name(B.swiglu_selected_variant(M, wl.N, wl.K)),
+             "us": round(f["us_median"], 2), "us_min": round(f["us_min"], 2), "cv": round(f["cv"], 4),
+             "tflops": round(fl / t / 1e12, 2), "gbs": round(by / t / 1e9, 1), "bound": bound,
+             "roofline_frac": round(t_roof / t, 4), "roofline_frac_nominal": round(t_nom / t, 4),
+             "roofline_frac_sustained": round(t_sus / t, 4),
+             "unfused_us": round(u["us_median"], 2),
+             "speedup_vs_unfused": round(u["us_median"] / f["us_median"], 3)}
+        if do_check:
+            p["parity"] = check_point(wl, M)
+        pts.append(p)
+    return pts
+
+
+# ---------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py executes oracle/)
+# ---------------------------------------------------------------------------------------
+_W_CACHE = {}
+
+
+def oracle_sample(name, rows, nthreads=0):
+    """Time the oracle, as it stands, on the first `rows` rows of the workload's largest batch
+    (all N columns, all of K).  Returns (seconds, flops, threads)."""
+    import oracle
+    from paper_2607_02521_b200 import inputs
+    table = dict(inputs.SHAPES)
+    table.update(inputs.PAPER_SHAPES)
+    K, N, seed, Ms = table[name]
+    if name not in _W_CACHE:
+        _W_CACHE[name] = inputs.make_weights(K, N, seed)
+        oracle.swiglu_oracle(inputs.make_activations(1, K, seed), *_W_CACHE[name], nthreads)
+    W1, W2 = _W_CACHE[name]
+    A = inputs.make_activations(rows, K, seed)
+    t0 = time.perf_counter()
+    _, used = oracle.swiglu_oracle(A, W1, W2, nthreads)
+    dt = time.perf_counter() - t0
+    return dt, flops(rows, N, K), used
+
+
+def cpu_baseline(name, target_s=12.0):
+    dt, fl, used = oracle_sample(name, 16)
+    rows = int(max(16, min(2048, 16 * target_s / max(dt, 1e-3))))
+    dt, fl, used = oracle_sample(name, rows)
+    table_rows = rows
+    return {"value": round(fl / dt / 1e12, 6), "unit": UNIT, "cores": used, "kind": "oracle",
+            "sample": f"{table_rows} rows x all N columns of {name} (fp64 oracle, "
+                      f"{fl / 1e9:.1f} GFLOP counted as 4MNK) in {dt:.2f} s",
+            "seconds": round(dt, 3)}
+
+
+def run_reference(args, ranks):
+    """--impl reference: this tier's reference arm is the CPU oracle, timed as it stands."""
+    if ranks.rank != 0:
+        return
+    name = args.workload
+    dt, fl, used = oracle_sample(name, 16)
+    rows = int(max(8, min(1024, 16 * (60.0 / max(1, args.steps + args.warmup)) / max(dt, 1e-3))))
+    times = []
+    for i in range(args.warmup + args.steps):
+        dt, fl, used = oracle_sample(name, rows)
+        if i >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * sum(times) / len(times)
+    value = fl / (ms * 1e-3) / 1e12
+    sample = f"{rows} rows x all N columns of {name} per step (fp64 CPU oracle)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": round(value, 6), "unit": UNIT,
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": round(ms, 3), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": name, "sample": sample},
+        "cpu_baseline": {"value": round(value, 6), "unit": UNIT, "cores": used,
+                         "kind": "oracle", "sample": sample},
+        "e2e": {"value": round(value, 6), "unit": UNIT, "h2d_bytes_per_step": 0,
+                "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ---------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------
+def read_traffic(name, M):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the
+    committed `ncu --set full` capture (profiles/traffic.json), or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(path)).get(f"{name}:M={M}")
+    except Exception:
+        return None
+
+
+def run_ours(args, ranks):
+    import numpy as np
+    import torch
+    from paper_2607_02521_b200 import binding as B
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(ranks.local_rank)
+    lib = B.load()
+    peaks, peak_src = load_peaks()
+    wl = Workload(args.workload, rank=ranks.rank)
+    order = sorted(wl.Ms, reverse=True)          # largest batch first: the host runs ahead
+    Mdom = order[0]
+    launches_per_step = sum(B.swiglu_launches_per_call(M, wl.N, wl.K) for M in order)
+
+    def step(ev=None):
+        for M in order:
+            if ev is not None and M == Mdom:
+                ev[0].record()
+                wl.call(lib.swiglu_mlp, M)
+                ev[1].record()
+            else:
+                wl.call(lib.swiglu_mlp, M)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    dom_events = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                  for _ in range(args.steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(ranks.local_rank).start()
+    ranks.barrier()
+    torch.cuda.synchronize()
+    e0.record()
+    for i in range(args.steps):
+        step(dom_events[i])
+    e1.record()
+    torch.cuda.synchronize()
+    ranks.barrier()
+    clocks = sampler.stop()
+    ms_total = ranks.max_over_ranks(e0.elapsed_time(e1))
+    ms_per_step = ms_total / args.steps
+    value = wl.flops_per_step() * ranks.world / (ms_per_step * 1e-3) / 1e12
+    dom_ms = statistics.mean(a.elapsed_time(b) for a, b in dom_events)
+
+    # roofline of the dominant kernel (the largest-M call: a dense bf16 contraction)
+    t_roof, bound = roofline_time_s(Mdom, wl.N, wl.K, peaks["bf16_tflops"], peaks["hbm_gbs"])
+    if bound == "tensor":
+        achieved, peak, runit = flops(Mdom, wl.N, wl.K) / (dom_ms * 1e-3) / 1e12, peaks["bf16_tflops"], "TFLOP/s"
+    else:
+        achieved, peak, runit = algo_bytes(Mdom, wl.N, wl.K) / (dom_ms * 1e-3) / 1e9, peaks["hbm_gbs"], "GB/s"
+    roofline = {"bound": bound, "achieved": round(achieved, 2), "peak": peak, "unit": runit,
+                "frac": round(achieved / peak, 4), "traffic": read_traffic(wl.name, Mdom),
+                "kernel": B.swiglu_variant_name(B.swiglu_selected_variant(Mdom, wl.N, wl.K)),
+                "M": Mdom, "us_per_launch": round(dom_ms * 1e3, 2),
+                "peak_source": f"{peak_src} (MEASURED_PEAKS.json burst figure)" if peak_src == "measured"
+                               else "fallback (B200_PROFILING.md)",
+                "frac_of_sustained": round(achieved / peaks["bf16_tflops_sustained"], 4) if bound == "tensor" else None,
+                "frac_of_nominal": round(achieved / (NOMINAL["bf16_tflops"] if bound == "tensor" else NOMINAL["hbm_gbs"]), 4)}
+
+    # end to end through the C ABI with HOST buffers (pinned): H2D + kernel + D2H every call
+    pin = lambda a: torch.from_numpy(a.view(np.int16)).pin_memory()
+    hA, hW1, hW2 = pin(wl.Ah), pin(wl.W1h), pin(wl.W2h)
+    hY = torch.empty((wl.Mmax, wl.N), dtype=torch.int16).pin_memory()
+    stream = torch.cuda.current_stream().cuda_stream
+
+    def e2e_step():
+        for M in order:
+            rc = lib.swiglu_mlp_host(hA.data_ptr(), hW1.data_ptr(), hW2.data_ptr(), hY.data_ptr(),
+                                     M, wl.N, wl.K, 0, stream)
+            if rc:
+                raise B.SwigluError(rc, B.last_error())
+
+    e2e_steps = max(1, min(args.steps, 10))
+    e2e_step()
+    ranks.barrier()
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(e2e_steps):
+        e2e_step()
+    e1.record()
+    torch.cuda.synchronize()
+    ranks.barrier()
+    e2e_ms = ranks.max_over_ranks(e0.elapsed_time(e1)) / e2e_steps
+    h2d = sum(M * wl.K * 2 + 2 * wl.K * wl.N * 2 for M in order)
+    d2h = sum(M * wl.N * 2 for M in order)
+    e2e = {"value": round(wl.flops_per_step() * ranks.world / (e2e_ms * 1e-3) / 1e12, 3), "unit": UNIT,
+           "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": round(e2e_ms, 3),
+           "steps": e2e_steps, "api": "swiglu_mlp_host (pinned host buffers)"}
+
+    points, cpu = None, None
+    if ranks.rank == 0:
+        if not args.no_points:
+            points = measure_points(wl, peaks, do_check=not args.no_check)
+        if ranks.world == 1 and not args.no_cpu_baseline:
+            cpu = cpu_baseline(wl.name)
+    ranks.barrier()
+    if ranks.rank != 0:
+        return
+    out = {
+        "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": ranks.world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 4),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic",
+        "config": {"workload": f"{wl.name}: K={wl.K}, N={wl.N}, one swiglu_mlp call per M in {order}",
+                   "l2": wl.l2_note, "parallelism": f"replicas x{ranks.world} (no collective)",
+                   "flops_per_step": wl.flops_per_step()},
+        "clocks": clocks, "roofline": roofline, "e2e": e2e,
+        "gpu_launches": launches_per_step * args.steps,
+    }
+    if cpu is not None:
+        out["cpu_baseline"] = cpu
+    if points is not None:
+        out["points"] = points
+    print(json.dumps(out))
+
+
+def run_all(args):
+    """Every BASELINE.json point (and, with --paper-grid, the paper's own grid) -> a table."""
+    import torch
+    from paper_2607_02521_b200 import inputs
+    peaks, peak_src = load_peaks()
+    names = list(inputs.SHAPES) + (list(inputs.PAPER_SHAPES) if args.paper_grid else [])
+    if args.only:
+        names = [n for n in names if n in args.only.split(",")]
+    sampler = ClockSampler(0).start()
+    pts = []
+    for name in names:
+        wl = Workload(name)
+        pts += measure_points(wl, peaks, do_check=not args.no_check)
+        del wl
+        torch.cuda.empty_cache()
+    clocks = sampler.stop()
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    json.dump({"peaks": peaks, "peak_source": peak_src, "clocks": clocks, "points": pts},
+              open(os.path.join(ROOT, "gpurun_out", "results.json"), "w"), indent=1)
+    hdr = ("| workload | M | variant | us | TFLOP/s | GB/s | bound | % of measured roofline | "
+           "% of nominal | unfused us | speed-up | mismatches fused / unfused (checked) |")
+    lines = [hdr, "|" + "---|" * 12]
+    for p in pts:
+        par = p.get("parity")
+        ptxt = (f"{par['fused']['mismatches']} / {par['unfused']['mismatches']} ({par['fused']['checked']})"
+                if par else "-")
+        lines.append(f"| {p['workload']} | {p['M']} | {p['variant']} | {p['us']} | {p['tflops']} | "
+                     f"{p['gbs']} | {p['bound']} | {100 * p['roofline_frac']:.1f} | "
+                     f"{100 * p['roofline_frac_nominal']:.1f} | {p['unfused_us']} | "
+                     f"{p['speedup_vs_unfused']} | {ptxt} |")
+    md = "\n".join(lines)
+    open(os.path.join(ROOT, "gpurun_out", "results.md"), "w").write(md + "\n")
+    print(md)
+    print(json.dumps({"clocks": clocks, "peak_source": peak_src}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="qwen2.5-1.5b")
+    ap.add_argument("--all", action="store_true")
+    ap.add_argument("--paper-grid", action="store_true")
+    ap.add_argument("--only", default="")
+    ap.add_argument("--no-points", action="store_true")
+    ap.add_argument("--no-check", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    from paper_2607_02521_b200.dist import Ranks
+    if args.impl == "reference":
+        rank = int(os.environ.get("RANK", "0"))
+        if rank != 0:
+            return                      # rank 0 alone runs the CPU oracle
+        class _Solo:
+            rank, world, local_rank = 0, 1, 0
+        run_reference(args, _Solo())
+        return
+    if args.all:
+        run_all(args)
+        return
+    ranks = Ranks()
+    if ranks.world != args.gpus and ranks.rank == 0:
+        print(f"note: --gpus {args.gpus} but WORLD_SIZE={ranks.world}; launch with torchrun",
+              file=sys.stderr)
+    try:
+        run_ours(args, ranks)
+    finally:
+        ranks.close()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,83 @@
+"""Multi-GPU plumbing for the bench: one process per GPU, no data-path collective.
+
+The path shards with independent units and no exchange step: each
+rank owns a replica of W1/W2 and its own batch of rows, so `--gpus N` is weak scaling and
+torch.distributed is used only for the barrier around the timed region and the
+max-over-ranks of the device time (NCCL on GPUs, gloo in the CPU tests).
+"""
+from __future__ import annotations
+
+import os
+
+
+class Ranks:
+    """torch.distributed wrapper that degrades to a single process when WORLD_SIZE is 1."""
+
+    def __init__(self, backend: str | None = None):
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+        self.dist = None
+        self.device = None
+        if self.world > 1:
+            import torch
+            import torch.distributed as dist
+            if backend is None:
+                backend = "nccl" if torch.cuda.is_available() else "gloo"
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29500")
+            if backend == "nccl":
+                torch.cuda.set_device(self.local_rank)
+                self.device = torch.device("cuda", self.local_rank)
+            dist.init_process_group(backend=backend, rank=self.rank, world_size=self.world)
+            self.dist = dist
+
+    def barrier(self) -> None:
+        if self.dist is not None:
+            self.dist.barrier()
+
+    def max_over_ranks(self, value: float) -> float:
+        """Slowest rank's time: what a multi-GPU number must be quoted on."""
+        if self.dist is None:
+            return float(value)
+        import torch
+        t = torch.tensor([float(value)], dtype=torch.float64,
+                         device=self.device if self.device is not None else "cpu")
+        if t.is_cuda:
+            t = t.float()
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(self, value: float) -> float:
+        if self.dist is None:
+            return float(value)
+        import torch
+        t = torch.tensor([float(value)], dtype=torch.float64,
+                         device=self.device if self.device is not None else "cpu")
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM)
+        return float(t.item())
+
+    def close(self) -> None:
+        if self.dist is not None:
+            self.dist.destroy_process_group()
+            self.dist = None
+
+
+def rank_seed_offset(rank: int) -> int:
+    """Each rank draws its OWN batch of rows (weights are replicated): rows of rank r are the
+    slice [r*M, (r+1)*M) of the shape's activation stream, so N ranks process N*M distinct
+    rows of the same workload."""
+    return int(rank)
+
+
+def shard_rows(total_rows: int, world: int, rank: int):
+    """Contiguous, balanced row ranges for splitting ONE global batch across ranks (the
+    strong-scaling form; rows are independent, Eq. 1-3 act row-wise)."""
+    base, extra = divmod(int(total_rows), int(world))
+    lo = rank * base + min(rank, extra)
+    return lo, lo + base + (1 if rank < extra else 0)
+
+
+def whole_job_throughput(units_per_rank: float, world: int, slowest_seconds: float) -> float:
+    """value = units all ranks processed / max-over-ranks time."""
+    return units_per_rank * world / slowest_seconds
