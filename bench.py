@@ -302,7 +302,8 @@ def run_reference(args, ranks):
         return
     name = args.workload
     dt, fl, used = oracle_sample(name, 16)
-    rows = int(max(8, min(1024, 16 * (60.0 / max(1, args.steps + args.warmup)) / max(dt, 1e-3))))
+    budget_s = float(os.environ.get("SWIGLU_REFERENCE_BUDGET_S", "60"))   # whole run, CPU seconds
+    rows = int(max(8, min(1024, 16 * (budget_s / max(1, args.steps + args.warmup)) / max(dt, 1e-3))))
     times = []
     for i in range(args.warmup + args.steps):
         dt, fl, used = oracle_sample(name, rows)
@@ -328,13 +329,18 @@ def run_reference(args, ranks):
 # our arm
 # ---------------------------------------------------------------------------------------
 def read_traffic(name, M):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the
-    committed `ncu --set full` capture (profiles/traffic.json), or None."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, copied
+    from the committed `ncu --set full` capture (profiles/traffic.csv names its source), or
+    None when that (workload, M) has not been captured."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
-        return json.load(open(path)).get(f"{name}:M={M}")
+        for row in csv.DictReader(open(path)):
+            if row["workload"] == name and int(row["M"]) == int(M):
+                return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 def run_ours(args, ranks):
