@@ -1,18 +1,24 @@
-// smallm_swiglu_kernel.cuh -- decode-sized batches (M <= 64): weight streaming is the whole
+// smallm_swiglu_kernel.cuh -- decode-sized batches (M <= 128): weight streaming is the whole
 // cost (bytes ~ 4*K*N, AI ~ M FLOP/B), so the kernel is built around HBM, not the tensor pipe.
 //
 //  * swap-AB: the 128-row UMMA operand is a W tile (128 output columns n, MN-major as W is
-//    [K,N] row-major), the narrow UMMA-N operand is A (MP = 16/32/64 padded tokens, K-major).
-//    Accumulators are Gate^T and Up^T: TMEM lane = n, column = m.  All 128 epilogue threads
-//    have work even at M = 1.
+//    [K,N] row-major), the narrow UMMA-N operand is A (MP = 16/32/64/128 padded tokens,
+//    K-major).  Accumulators are Gate^T and Up^T: TMEM lane = n, column = m.  All 128
+//    epilogue threads have work even at M = 1.
 //  * split-K over a thread-block cluster: the S CTAs of a cluster share one 128-column tile
-//    and each streams 1/S of K, so ~150-300 CTAs stream equal bytes whatever N/128 is.
+//    and each streams 1/S of K, so every SM streams equal bytes whatever N/128 is.
 //    SiLU is non-linear, so partial Gate/Up sums are reduced BEFORE the activation: each CTA
 //    parks its fp32 partials in its own shared memory, and after a cluster barrier CTA r sums
 //    rows m = r, r+S, ... over all peers through distributed shared memory in rank order
-//    (deterministic), applies SiLU-multiply and stores bf16.  No global workspace, Gate/Up
-//    never reach HBM (BASELINE.json north_star "Small M").
-//  * two CTAs per SM, 3-stage TMA ring each (~200 KB of loads in flight per SM).
+//    (deterministic; all 2S loads of a row are in flight together), applies SiLU-multiply and
+//    stores bf16, 8 bytes per thread, 256 contiguous bytes per warp.  No global workspace,
+//    Gate/Up never reach HBM (BASELINE.json north_star "Small M").
+//  * fixed costs matter at these sizes (a call is 3-15 us): the producer thread initialises
+//    its barriers and issues the first ring of TMA loads BEFORE the CTA-wide setup barrier
+//    (TMEM allocation overlaps the HBM latency of the first loads), and warp 0 issues L2
+//    prefetches for the CTA's weight blocks before griddepcontrol.wait, so under programmatic
+//    dependent launch the weights start moving while the previous kernel drains.  A prefetch
+//    is a hint: it cannot observe or produce stale data (L2 is the point of coherence).
 #pragma once
 #include <cuda.h>
 
@@ -20,12 +26,14 @@
 
 namespace swiglu {
 
-constexpr int kSmallMMax = 64;
+constexpr int kSmallMMax = 128;
 constexpr int kSmallThreads = 192;  // warp 0 TMA, warp 1 MMA, warps 2-5 epilogue
+constexpr int kSmallPrefetchMax = 32;     // k-blocks per CTA prefetched to L2 (one per lane)
 
 template <int MP>
 struct SmallCfg {
-  static constexpr int kStages = (MP <= 32) ? 3 : 2;
+  static constexpr int kCtasPerSm = (MP <= 64) ? 2 : 1;
+  static constexpr int kStages = (MP <= 32) ? 3 : (MP == 64 ? 2 : 4);
   static constexpr int kWBytes = 128 * BK * 2;  // one W tile: 128 n x 64 k = 16 KB
   static constexpr int kABytes = MP * BK * 2;   // MP tokens x 64 k
   static constexpr int kStageBytes = 2 * kWBytes + kABytes;
@@ -38,17 +46,33 @@ struct SmallCfg {
 struct SmallParams {
   int M, N, K;
   int ksplit;         // cluster size S
+  int prefetch_blocks;  // leading k-blocks of each CTA's weight stream to prefetch into L2
   long long ldy;      // = N
+#ifdef SWIGLU_TRACE
+  unsigned long long* trace;  // [grid][16] globaltimer stamps (debug builds only)
+#endif
 };
 
-__device__ __forceinline__ float ld_dsmem_f32(uint32_t cluster_addr) {
-  float v;
-  asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(cluster_addr) : "memory");
+#ifdef SWIGLU_TRACE
+#define SWIGLU_TRACE_POINT(i)                                                         \
+  do {                                                                                \
+    if (p.trace) p.trace[(size_t)blockIdx.x * 16 + (i)] = globaltimer_ns();           \
+  } while (0)
+#else
+#define SWIGLU_TRACE_POINT(i) do { } while (0)
+#endif
+
+__device__ __forceinline__ float4 ld_dsmem_v4(uint32_t cluster_addr) {
+  float4 v;
+  asm volatile("ld.shared::cluster.v4.f32 {%0, %1, %2, %3}, [%4];"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+               : "r"(cluster_addr)
+               : "memory");
   return v;
 }
 
 template <int MP>
-__global__ void __launch_bounds__(kSmallThreads, 2)
+__global__ void __launch_bounds__(kSmallThreads, SmallCfg<MP>::kCtasPerSm)
 smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                      const __grid_constant__ CUtensorMap tmap_w1,
                      const __grid_constant__ CUtensorMap tmap_w2, uint16_t* __restrict__ Y,
@@ -76,42 +100,65 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   const int kb_begin = (int)(((long long)k_blocks * rank) / S);
   const int kb_end = (int)(((long long)k_blocks * (rank + 1)) / S);
 
-  if (warp == 0 && lane == 0) {
-    prefetch_tensormap(&tmap_a);
-    prefetch_tensormap(&tmap_w1);
-    prefetch_tensormap(&tmap_w2);
-    for (int s = 0; s < kStages; ++s) {
-      mbar_init(full_bar(s), 1);
-      mbar_init(empty_bar(s), 1);
+  auto issue_stage = [&](int kb, int s) {
+    const uint32_t fb = full_bar(s);
+    mbar_arrive_expect_tx(fb, Cfg::kStageBytes);
+    const int k0 = kb * BK;
+    // weights are read exactly once per call: do not let them push A out of L2
+    tma_load_2d(smem_w1(s), &tmap_w1, fb, n_base, k0, kEvictFirst);
+    tma_load_2d(smem_w1(s) + 8192, &tmap_w1, fb, n_base + 64, k0, kEvictFirst);
+    tma_load_2d(smem_w2(s), &tmap_w2, fb, n_base, k0, kEvictFirst);
+    tma_load_2d(smem_w2(s) + 8192, &tmap_w2, fb, n_base + 64, k0, kEvictFirst);
+    tma_load_2d(smem_act(s), &tmap_a, fb, k0, 0, kEvictLast);
+  };
+
+  if (threadIdx.x == 0) SWIGLU_TRACE_POINT(0);
+  // ------------------------------------------------------------------ setup
+  if (warp == 0) {
+    if (lane == 0) {
+      prefetch_tensormap(&tmap_w1);
+      prefetch_tensormap(&tmap_w2);
+      prefetch_tensormap(&tmap_a);
+      for (int s = 0; s < kStages; ++s) {
+        mbar_init(full_bar(s), 1);
+        mbar_init(empty_bar(s), 1);
+      }
+      mbar_init(acc_full_bar, 1);
+      fence_mbar_init();
+      fence_proxy_async_all();
     }
-    mbar_init(acc_full_bar, 1);
-    fence_mbar_init();
+    // L2 prefetch of this CTA's weight stream (hint; legal before griddepcontrol.wait)
+    const int kb = kb_begin + (int)lane;
+    if ((int)lane < p.prefetch_blocks && kb < kb_end) {
+      tma_prefetch_l2_2d(&tmap_w1, n_base, kb * BK);
+      tma_prefetch_l2_2d(&tmap_w1, n_base + 64, kb * BK);
+      tma_prefetch_l2_2d(&tmap_w2, n_base, kb * BK);
+      tma_prefetch_l2_2d(&tmap_w2, n_base + 64, kb * BK);
+    }
+    if (lane == 0) {
+      // A may be the previous kernel's output: real loads only after the grid dependency
+      pdl_wait_prior_grid();
+      SWIGLU_TRACE_POINT(2);
+      for (int i = 0; i < kStages && kb_begin + i < kb_end; ++i) issue_stage(kb_begin + i, i);
+    }
+  } else if (warp == 1) {
+    tmem_alloc<1>(tmem_slot, Cfg::kTmemCols);
   }
-  if (warp == 1) tmem_alloc<1>(tmem_slot, Cfg::kTmemCols);
   tcgen05_fence_before();
   __syncthreads();
   tcgen05_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
-
-  pdl_wait_prior_grid();
   pdl_launch_dependents();
+  if (threadIdx.x == 0) SWIGLU_TRACE_POINT(1);
 
   if (warp == 0 && lane == 0) {
-    // ================================================================ TMA producer
+    // ================================================================ TMA producer (rest)
     int s = 0;
-    uint32_t ph = 0;
-    for (int kb = kb_begin; kb < kb_end; ++kb) {
+    uint32_t ph = 1;  // the first kStages blocks went out above; now on the ring's second lap
+    for (int kb = kb_begin + kStages; kb < kb_end; ++kb) {
       mbar_wait(empty_bar(s), ph ^ 1u);
-      const uint32_t fb = full_bar(s);
-      mbar_arrive_expect_tx(fb, Cfg::kStageBytes);
-      const int k0 = kb * BK;
-      // weights are read exactly once per call: do not let them push A out of L2
-      tma_load_2d(smem_w1(s), &tmap_w1, fb, n_base, k0, kEvictFirst);
-      tma_load_2d(smem_w1(s) + 8192, &tmap_w1, fb, n_base + 64, k0, kEvictFirst);
-      tma_load_2d(smem_w2(s), &tmap_w2, fb, n_base, k0, kEvictFirst);
-      tma_load_2d(smem_w2(s) + 8192, &tmap_w2, fb, n_base + 64, k0, kEvictFirst);
-      tma_load_2d(smem_act(s), &tmap_a, fb, k0, 0, kEvictLast);
+      issue_stage(kb, s);
       if (++s == kStages) { s = 0; ph ^= 1u; }
     }
   } else if (warp == 1 && lane == 0) {
@@ -121,6 +168,7 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     uint32_t ph = 0;
     for (int kb = kb_begin; kb < kb_end; ++kb) {
       mbar_wait(full_bar(s), ph);
+      if (kb == kb_begin) SWIGLU_TRACE_POINT(3);
       tcgen05_fence_after();
 #pragma unroll
       for (int k = 0; k < BK / UMMA_K; ++k) {
@@ -137,23 +185,27 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       if (++s == kStages) { s = 0; ph ^= 1u; }
     }
     umma_commit<1>(acc_full_bar);
+    SWIGLU_TRACE_POINT(4);
   }
 
   // ================================================================ epilogue
-  const uint32_t q = warp & 3u;
-  const uint32_t nl = q * 32u + lane;  // local output column = TMEM lane
-  const int n = n_base + (int)nl;
-  const uint32_t part = smem_base;     // fp32 [2][MP][128], aliases the (drained) ring
+  // 1. park this CTA's partial Gate^T / Up^T (fp32 [2][MP][128], n contiguous) in the drained ring
+  const uint32_t part = smem_base;
   if (warp >= 2) {
-    if (kb_end > kb_begin) {
+    const uint32_t q = warp & 3u;
+    const uint32_t nl = q * 32u + lane;  // local output column = TMEM lane
+    const bool have = kb_end > kb_begin;
+    if (have) {
       mbar_wait(acc_full_bar, 0);
       tcgen05_fence_after();
     }
+    if (threadIdx.x == 64) SWIGLU_TRACE_POINT(5);
     const uint32_t tacc = tmem_base + ((q * 32u) << 16);
 #pragma unroll
     for (int c = 0; c < MP / 16; ++c) {
+      if (c * 16 >= p.M) break;  // rows >= M are never read back
       uint32_t g[16], u[16];
-      if (kb_end > kb_begin) {
+      if (have) {
         tmem_ld_32x32b_x16(tacc + c * 16, g);
         tmem_ld_32x32b_x16(tacc + MP + c * 16, u);
         tmem_ld_wait();
@@ -161,50 +213,73 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
 #pragma unroll
         for (int j = 0; j < 16; ++j) g[j] = u[j] = 0u;  // this rank got no k-blocks
       }
-      if (S == 1) {
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          const int m = c * 16 + j;
-          if (m < p.M && n < p.N) {
-            const float y = silu_mul(__uint_as_float(g[j]), __uint_as_float(u[j]));
-            Y[(long long)m * p.ldy + n] = (uint16_t)(pack_bf16x2_rn(y, 0.f) & 0xFFFFu);
-          }
-        }
-      } else {
+      for (int j = 0; j < 16; ++j) {
+        const int m = c * 16 + j;
+        asm volatile("st.shared.b32 [%0], %1;" ::"r"(part + (uint32_t)(m * 128 + nl) * 4u),
+                     "r"(g[j]) : "memory");
+        asm volatile("st.shared.b32 [%0], %1;" ::"r"(part + (uint32_t)((MP + m) * 128 + nl) * 4u),
+                     "r"(u[j]) : "memory");
+      }
+    }
+    tcgen05_fence_before();
+  }
+  // 2. all partials of the cluster are in place
+  if (S > 1) {
+    __syncwarp();
+    cluster_sync();
+  } else {
+    __syncthreads();
+  }
+  if (threadIdx.x == 64) SWIGLU_TRACE_POINT(6);
+  // 3. rank r reduces rows m = r, r+S, ... over all peers (fixed rank order), SiLU-mul, store
+  if (warp >= 2) {
+    pdl_wait_prior_grid();  // Y may still be being written by the previous kernel in the stream
+    const uint32_t et = threadIdx.x - 64u;
+    const uint32_t c4 = (et & 31u) * 4u;  // 4 consecutive output columns per thread
+    const uint32_t sub = et >> 5;         // 4 rows in flight per pass
+    const int n = n_base + (int)c4;
+    uint32_t peer[8];
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          const int m = c * 16 + j;
-          asm volatile("st.shared.b32 [%0], %1;" ::"r"(part + (uint32_t)(m * 128 + nl) * 4u),
-                       "r"(g[j]) : "memory");
-          asm volatile("st.shared.b32 [%0], %1;" ::"r"(part + (uint32_t)((MP + m) * 128 + nl) * 4u),
-                       "r"(u[j]) : "memory");
+    for (int r = 0; r < 8; ++r) peer[r] = (r < S) ? mapa_shared(part, (uint32_t)r) : 0u;
+    for (int m = (int)rank + S * (int)sub; m < p.M; m += 4 * S) {
+      const uint32_t goff = (uint32_t)(m * 128 + (int)c4) * 4u;
+      const uint32_t uoff = (uint32_t)((MP + m) * 128 + (int)c4) * 4u;
+      float4 g[8], u[8];
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        if (r < S) {
+          g[r] = ld_dsmem_v4(peer[r] + goff);
+          u[r] = ld_dsmem_v4(peer[r] + uoff);
         }
+      }
+      float4 gs = g[0], us = u[0];
+#pragma unroll
+      for (int r = 1; r < 8; ++r) {
+        if (r < S) {
+          gs.x += g[r].x; gs.y += g[r].y; gs.z += g[r].z; gs.w += g[r].w;
+          us.x += u[r].x; us.y += u[r].y; us.z += u[r].z; us.w += u[r].w;
+        }
+      }
+      if (n < p.N) {  // N % 8 == 0 and n % 4 == 0: the 4 columns are in range together
+        const uint32_t lo = pack_bf16x2_rn(silu_mul(gs.x, us.x), silu_mul(gs.y, us.y));
+        const uint32_t hi = pack_bf16x2_rn(silu_mul(gs.z, us.z), silu_mul(gs.w, us.w));
+        *reinterpret_cast<uint2*>(Y + (long long)m * p.ldy + n) = make_uint2(lo, hi);
       }
     }
   }
-  __syncwarp();
+  if (threadIdx.x == 64) SWIGLU_TRACE_POINT(7);
   if (S > 1) {
-    cluster_sync();  // every CTA's partials are in its shared memory
-    if (warp >= 2) {
-      for (int m = (int)rank; m < p.M; m += S) {
-        float gs = 0.f, us = 0.f;
-        for (int r = 0; r < S; ++r) {  // fixed rank order: run-to-run deterministic
-          gs += ld_dsmem_f32(mapa_shared(part + (uint32_t)(m * 128 + nl) * 4u, r));
-          us += ld_dsmem_f32(mapa_shared(part + (uint32_t)((MP + m) * 128 + nl) * 4u, r));
-        }
-        if (n < p.N)
-          Y[(long long)m * p.ldy + n] = (uint16_t)(pack_bf16x2_rn(silu_mul(gs, us), 0.f) & 0xFFFFu);
-      }
-    }
     __syncwarp();
     cluster_sync();  // peers may still be reading this CTA's partials
+  } else {
+    __syncthreads();
   }
-  tcgen05_fence_before();
-  __syncthreads();
   if (warp == 1) {
     tcgen05_fence_after();
     tmem_dealloc<1>(tmem_base, Cfg::kTmemCols);
   }
+  if (threadIdx.x == 0) SWIGLU_TRACE_POINT(8);
 }
 
 }  // namespace swiglu

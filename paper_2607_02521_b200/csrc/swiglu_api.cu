@@ -39,7 +39,7 @@ int fail_cuda(cudaError_t e, const char* what) {
 enum FusedVariant {
   kFused1Cta = 0,     // 128x128 (Gate|Up) tile per CTA
   kFused2Cta = 1,     // 256x128 tile per CTA pair, cta_group::2
-  kFusedSmallM = 2,   // swap-AB, split-K over a cluster, for M <= 64
+  kFusedSmallM = 2,   // swap-AB, split-K over a cluster, for M <= 128
   kNumFused = 3
 };
 enum UnfusedVariant { kUnfused1Cta = 0, kUnfused2Cta = 1, kNumUnfused = 2 };
@@ -55,13 +55,18 @@ int env_int(const char* name, int dflt) {
 
 // Measured dispatch (table regenerated from bench sweeps).
 int select_fused(int64_t M, int64_t N, int64_t K) {
-  (void)N; (void)K;
+  (void)K;
   const int forced = env_int("SWIGLU_VARIANT", -1);
   if (forced >= 0 && forced < kNumFused) {
     if (forced != kFusedSmallM || M <= swiglu::kSmallMMax) return forced;
   }
-  if (M <= swiglu::kSmallMMax) return kFusedSmallM;
-  if (M <= 128) return kFused1Cta;
+  if (M <= 64) return kFusedSmallM;
+  if (M <= 128) {
+    // HBM-bound either way; the 1-CTA kernel has one CTA per 128-column tile, so with fewer
+    // tiles than ~3/4 of the 148 SMs the split-K kernel (all SMs streaming) wins.
+    const int64_t n_tiles = (N + 127) / 128;
+    return (n_tiles * 4 <= 148 * 3) ? kFusedSmallM : kFused1Cta;
+  }
   return kFused2Cta;
 }
 int select_unfused(int64_t M, int64_t N, int64_t K) {
@@ -168,6 +173,9 @@ int get_device_state(DeviceState** out) {
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64>,
                                   cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   SmallCfg<64>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<128>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  SmallCfg<128>::kSmemBytes));
     d.ready = true;
   }
   *out = &d;
@@ -191,6 +199,10 @@ int make_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
                 (int)r, (long long)inner, (long long)outer);
   return SWIGLU_OK;
 }
+
+#ifdef SWIGLU_TRACE
+unsigned long long* g_trace = nullptr;  // debug builds: device buffer for globaltimer stamps
+#endif
 
 bool pdl_enabled() {
   static const bool on = env_int("SWIGLU_NO_PDL", 0) == 0;
@@ -251,11 +263,11 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   return SWIGLU_OK;
 }
 
-// Split-K factor of the small-M kernel: as many CTAs as can be co-resident (2 per SM), at
-// most 8 per cluster (portable cluster size), at least one k-block per CTA.
-int smallm_ksplit(int sm_count, int64_t n_tiles, int64_t k_blocks) {
+// Split-K factor of the small-M kernel: as many CTAs as can be co-resident, at most 8 per
+// cluster (portable cluster size), at least one k-block per CTA.
+int smallm_ksplit(int sm_count, int ctas_per_sm, int64_t n_tiles, int64_t k_blocks) {
   const int forced = env_int("SWIGLU_KSPLIT", 0);
-  int64_t s = (2ll * sm_count) / n_tiles;
+  int64_t s = ((int64_t)ctas_per_sm * sm_count) / n_tiles;
   if (forced > 0) s = forced;
   if (s > 8) s = 8;
   if (s > k_blocks) s = k_blocks;
@@ -275,8 +287,17 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   const int64_t n_tiles = (N + 127) / 128, k_blocks = (K + BK - 1) / BK;
   SmallParams p;
   p.M = (int)M; p.N = (int)N; p.K = (int)K;
-  p.ksplit = smallm_ksplit(d.sm_count, n_tiles, k_blocks);
+  p.ksplit = smallm_ksplit(d.sm_count, SmallCfg<MP>::kCtasPerSm, n_tiles, k_blocks);
   p.ldy = N;
+  // L2 prefetch ahead of the grid dependency: at most ~32 MiB over the whole grid
+  const int64_t grid = n_tiles * p.ksplit;
+  int64_t pf = (32ll << 20) / (grid * 2 * SmallCfg<MP>::kWBytes);
+  if (pf > kSmallPrefetchMax) pf = kSmallPrefetchMax;
+  if (env_int("SWIGLU_NO_PREFETCH", 0)) pf = 0;
+  p.prefetch_blocks = (int)pf;
+#ifdef SWIGLU_TRACE
+  p.trace = g_trace;
+#endif
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof cfg);
   cfg.gridDim = dim3((unsigned)(n_tiles * p.ksplit));
@@ -307,7 +328,8 @@ int launch_smallm(const DeviceState& d, const void* A, const void* W1, const voi
                   int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
   if (M <= 16) return launch_smallm_mp<16>(d, A, W1, W2, Y, M, N, K, stream);
   if (M <= 32) return launch_smallm_mp<32>(d, A, W1, W2, Y, M, N, K, stream);
-  return launch_smallm_mp<64>(d, A, W1, W2, Y, M, N, K, stream);
+  if (M <= 64) return launch_smallm_mp<64>(d, A, W1, W2, Y, M, N, K, stream);
+  return launch_smallm_mp<128>(d, A, W1, W2, Y, M, N, K, stream);
 }
 
 int launch_silu_mul(const DeviceState& d, const void* G, const void* U, void* Y, int64_t elems,
@@ -514,6 +536,10 @@ int swiglu_mlp_host(const void* A_host, const void* W1_host, const void* W2_host
   CUDA_TRY(cudaStreamSynchronize(stream));
   return SWIGLU_OK;
 }
+
+#ifdef SWIGLU_TRACE
+void swiglu_debug_set_trace(void* device_buffer) { g_trace = (unsigned long long*)device_buffer; }
+#endif
 
 const char* swiglu_last_error(void) { return g_err; }
 

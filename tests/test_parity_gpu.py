@@ -81,15 +81,28 @@ def test_large_m_kernels_on_odd_shapes(kind, variant, M, N, K):
 
 @pytest.mark.parametrize("M,N,K", [(1, 128, 64), (1, 8960, 1536), (7, 136, 72), (16, 4864, 896),
                                    (17, 392, 328), (32, 1160, 896), (33, 264, 200),
-                                   (64, 4864, 896), (5, 29568, 512)])
+                                   (64, 4864, 896), (5, 29568, 512), (65, 264, 200),
+                                   (100, 1160, 328), (128, 4864, 896), (127, 8960, 1536),
+                                   (128, 128, 64), (3, 8, 8), (48, 136, 8)])
 def test_small_m_kernel_on_odd_shapes(M, N, K):
     A, W1, W2 = inputs.make_case(M, N, K, seed=200 + M + N + K, std=0.05)
     y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
     assert_parity(run("fused", 2, A, W1, W2), y_ref, ("smallm", M, N, K))
 
 
+@pytest.mark.parametrize("ksplit", [1, 2, 3, 5, 8])
+@pytest.mark.parametrize("M", [1, 16, 40, 128])
+def test_small_m_kernel_every_cluster_size(M, ksplit, monkeypatch):
+    """Forced split-K factor (cluster size): the DSMEM reduction must give the same result
+    for any S, including S that does not divide the number of k-blocks or M."""
+    monkeypatch.setenv("SWIGLU_KSPLIT", str(ksplit))
+    A, W1, W2 = inputs.make_case(M, 520, 712, seed=300 + M, std=0.05)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+    assert_parity(run("fused", 2, A, W1, W2), y_ref, ("smallm", M, ksplit))
+
+
 def test_small_m_variant_rejects_large_m():
-    A, W1, W2 = inputs.make_case(65, 128, 64, seed=1)
+    A, W1, W2 = inputs.make_case(129, 128, 64, seed=1)
     with pytest.raises(B.SwigluError) as e:
         run("fused", 2, A, W1, W2)
     assert e.value.status == B.SWIGLU_ERR_UNSUPPORTED
