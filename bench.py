@@ -167,7 +167,7 @@ class ClockSampler:
 # workload: one (K, N) shape with its batch sizes, resident in HBM, weights rotating
 # ---------------------------------------------------------------------------------------
 class Workload:
-    def __init__(self, name, rank=0, rotate=True):
+    def __init__(self, name, rank=0, rotate=True, Ms=None):
         import numpy as np
         import torch
         from paper_2607_02521_b200 import inputs
@@ -175,6 +175,8 @@ class Workload:
         table.update(inputs.PAPER_SHAPES)
         self.name = name
         self.K, self.N, self.seed, self.Ms = table[name]
+        if Ms:
+            self.Ms = tuple(Ms)          # extra batch sizes for sweeps (same seeded streams)
         self.Mmax = max(self.Ms)
         K, N = self.K, self.N
         self.W1h, self.W2h = inputs.make_weights(K, N, self.seed)
@@ -237,7 +239,7 @@ def time_point(wl, fn, M, target_ms=1.5, batches=15):
     with torch.cuda.graph(g):
         for _ in range(per):
             wl.call(fn, M)
-    for _ in range(2):
+    for _ in range(max(2, int(10.0 / max(est_ms * per, 1e-3)))):   # ~10 ms of warm replays
         g.replay()
     torch.cuda.synchronize()
     samples = []
@@ -547,6 +549,63 @@ def run_all(args):
     print(json.dumps({"clocks": clocks, "peak_source": peak_src}))
 
 
+def run_sweep(args):
+    """Dispatch-table sweeps (`--sweep variants` / `--sweep ksplit`): time every fused variant
+    (forced through swiglu_mlp_ex) or every split-K factor of the small-M kernel
+    (SWIGLU_KSPLIT) per (shape, M), cold L2, CUDA-graph replay.  Writes a markdown table to
+    gpurun_out/sweep_<kind>.md; select_fused() / smallm_ksplit() in swiglu_api.cu are fitted
+    to these tables."""
+    import torch
+    from paper_2607_02521_b200 import binding as B, inputs
+    lib = B.load()
+    names = [n for n in inputs.SHAPES if not args.only or n in args.only.split(",")]
+    Ms = [int(m) for m in args.sweep_m.split(",")]
+    nvar = B.swiglu_num_variants()
+    lines = []
+    if args.sweep == "variants":
+        cols = ["auto"] + [B.swiglu_variant_name(v) for v in range(nvar)]
+        lines += ["| workload | M | " + " | ".join(cols) + " | auto picks |", "|---|---|" + "---|" * (len(cols) + 1)]
+    else:
+        ks = list(range(1, 9))
+        lines += ["| workload | M | " + " | ".join(f"S={k}" for k in ks) + " | auto (S) |", "|---|---|" + "---|" * 9]
+
+    def forced(v):
+        def fn(a, w1, w2, y, M, N, K, stream):
+            return lib.swiglu_mlp_ex(a, w1, w2, y, M, N, K, None, 0, v, stream)
+        return fn
+
+    for name in names:
+        wl = Workload(name, Ms=Ms)
+        for M in Ms:
+            cells = []
+            if args.sweep == "variants":
+                for v in [-1] + list(range(nvar)):
+                    try:
+                        cells.append(f"{time_point(wl, forced(v), M)['us_median']:.2f}")
+                    except B.SwigluError:
+                        cells.append("n/a")
+                pick = B.swiglu_variant_name(B.swiglu_selected_variant(M, wl.N, wl.K))
+            else:
+                small = [v for v in range(nvar) if "smallm" in B.swiglu_variant_name(v)][0]
+                for k in ks:
+                    os.environ["SWIGLU_KSPLIT"] = str(k)
+                    try:
+                        cells.append(f"{time_point(wl, forced(small), M)['us_median']:.2f}")
+                    except B.SwigluError:
+                        cells.append("n/a")
+                os.environ["SWIGLU_KSPLIT"] = "0"
+                try:
+                    pick = f"{time_point(wl, forced(small), M)['us_median']:.2f}"
+                except B.SwigluError:
+                    pick = "n/a"
+            lines.append(f"| {name} | {M} | " + " | ".join(cells) + f" | {pick} |")
+            print(lines[-1], flush=True)
+        del wl
+        torch.cuda.empty_cache()
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    open(os.path.join(ROOT, "gpurun_out", f"sweep_{args.sweep}.md"), "w").write("\n".join(lines) + "\n")
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -560,6 +619,8 @@ def main():
     ap.add_argument("--no-points", action="store_true")
     ap.add_argument("--no-check", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", default="", choices=["", "variants", "ksplit"])
+    ap.add_argument("--sweep-m", default="1,16,32,64,128,256")
     args = ap.parse_args()
     from paper_2607_02521_b200.dist import Ranks
     if args.impl == "reference":
@@ -572,6 +633,9 @@ def main():
         return
     if args.all:
         run_all(args)
+        return
+    if args.sweep:
+        run_sweep(args)
         return
     ranks = Ranks()
     if ranks.world != args.gpus and ranks.rank == 0:

@@ -28,19 +28,21 @@ using namespace sm100;
 constexpr int BM = 128;      // rows of A / Y per CTA
 constexpr int BK = 64;       // k per pipeline stage: 64 bf16 = one 128-byte swizzle row
 constexpr int UMMA_K = 16;   // k per tcgen05.mma (kind::f16)
-constexpr int UMMA_N = 256;  // accumulator columns per tile
 constexpr int kEpiWarps = 4;
 constexpr int kGemmThreads = 64 + 32 * kEpiWarps;  // warp 0 TMA, warp 1 MMA, warps 2-5 epilogue
-constexpr int kTmemCols = 512;                     // 2 accumulator stages x 256 columns
 constexpr int kOutBufBytes = BM * 64 * 2;          // one 64-column bf16 output chunk (16 KB)
 
-template <int kCtaGroup>
+// kUmmaN = accumulator columns per tile: 256 (fused: Gate 128 | Up 128; unfused: 256 plain
+// columns) or, for the narrow fused tile used when N/128 tiles cannot fill the GPU,
+// 128 (Gate 64 | Up 64).
+template <int kCtaGroup, int kUmmaN = 256>
 struct GemmCfg {
-  static constexpr int kBColsPerCta = UMMA_N / kCtaGroup;
+  static constexpr int kBColsPerCta = kUmmaN / kCtaGroup;
   static constexpr int kABytes = BM * BK * 2;            // 16 KB
-  static constexpr int kBBytes = kBColsPerCta * BK * 2;  // 32 KB (1-CTA) / 16 KB (2-CTA)
+  static constexpr int kBBytes = kBColsPerCta * BK * 2;  // 32 KB (1-CTA) / 16 KB (2-CTA, narrow)
   static constexpr int kStageBytes = kABytes + kBBytes;
-  static constexpr int kStages = (kCtaGroup == 1) ? 4 : 6;
+  static constexpr int kStages = (kStageBytes >= 48 * 1024) ? 4 : 6;
+  static constexpr int kTmemCols = 2 * kUmmaN;           // 2 accumulator stages
   static constexpr int kBarBytes = 1024;
   // +1024: slack to align the dynamic smem base to 1024 B (128-byte swizzle atoms)
   static constexpr int kSmemBytes = kStages * kStageBytes + 2 * kOutBufBytes + kBarBytes + 1024;
@@ -51,6 +53,7 @@ struct GemmParams {
   int m_tiles;   // ceil(M / (128*kCtaGroup))
   int n_tiles;   // ceil(N / (fused ? 128 : 256))
   int group_m;   // m-tiles per L2 raster group
+  int early_issue;      // 1: fill the ring before the CTA-wide setup barrier (small grids)
 };
 
 // Tile order: groups of `group_m` row-tiles x all column-tiles, row-tile fastest inside a
@@ -73,15 +76,18 @@ __device__ __forceinline__ float silu_mul(float g, float u) {
   return (g * u) * r;
 }
 
-template <int kCtaGroup, bool kFused>
+template <int kCtaGroup, bool kFused, int kBN = 128>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                    const __grid_constant__ CUtensorMap tmap_b1,
                    const __grid_constant__ CUtensorMap tmap_b2,
                    const __grid_constant__ CUtensorMap tmap_y, const GemmParams p) {
-  using Cfg = GemmCfg<kCtaGroup>;
+  static_assert(kBN == 128 || (kBN == 64 && kFused && kCtaGroup == 1), "narrow tile: fused 1-CTA");
+  constexpr int UMMA_N = kFused ? 2 * kBN : 256;  // accumulator columns per tile
+  using Cfg = GemmCfg<kCtaGroup, UMMA_N>;
   constexpr int kStages = Cfg::kStages;
-  constexpr int kOutCols = kFused ? 128 : 256;  // output columns per tile
+  constexpr int kTmemCols = Cfg::kTmemCols;
+  constexpr int kOutCols = kFused ? kBN : 256;  // output columns per tile
   constexpr int kChunks = kOutCols / 64;        // 64-column epilogue chunks per tile
 
   extern __shared__ uint8_t smem_raw[];
@@ -104,21 +110,72 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   const int total_tiles = p.m_tiles * p.n_tiles;
   const int k_blocks = (p.K + BK - 1) / BK;
 
+  // One k-block of A and B into ring slot s (no waiting here: the caller owns the ring state).
+  auto issue_loads = [&](int s, int kb, int m_base, int n_base) {
+    if (rank == 0) mbar_arrive_expect_tx(full_bar(s), Cfg::kStageBytes * kCtaGroup);
+    const int k0 = kb * BK;
+    const uint32_t sa = smem_a(s), sb = smem_b(s), fb = full_bar(s);
+    if constexpr (kCtaGroup == 1) {
+      tma_load_2d(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
+      if constexpr (kFused && kBN == 64) {
+        tma_load_2d(sb, &tmap_b1, fb, n_base, k0, kEvictNormal);
+        tma_load_2d(sb + 8192, &tmap_b2, fb, n_base, k0, kEvictNormal);
+      } else if constexpr (kFused) {
+        tma_load_2d(sb, &tmap_b1, fb, n_base, k0, kEvictNormal);
+        tma_load_2d(sb + 8192, &tmap_b1, fb, n_base + 64, k0, kEvictNormal);
+        tma_load_2d(sb + 16384, &tmap_b2, fb, n_base, k0, kEvictNormal);
+        tma_load_2d(sb + 24576, &tmap_b2, fb, n_base + 64, k0, kEvictNormal);
+      } else {
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          tma_load_2d(sb + j * 8192, &tmap_b1, fb, n_base + j * 64, k0, kEvictNormal);
+      }
+    } else {
+      tma_load_2d_pair(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
+      if constexpr (kFused) {
+        const CUtensorMap* tb = (rank == 0) ? &tmap_b1 : &tmap_b2;
+        tma_load_2d_pair(sb, tb, fb, n_base, k0, kEvictNormal);
+        tma_load_2d_pair(sb + 8192, tb, fb, n_base + 64, k0, kEvictNormal);
+      } else {
+        const int nb = n_base + (int)rank * 128;
+        tma_load_2d_pair(sb, &tmap_b1, fb, nb, k0, kEvictNormal);
+        tma_load_2d_pair(sb + 8192, &tmap_b1, fb, nb + 64, k0, kEvictNormal);
+      }
+    }
+  };
+  int pre = 0;  // k-blocks of this CTA's first tile issued before the setup barrier
+
   // ------------------------------------------------------------------ one-time setup
-  if (warp == 0 && lane == 0) {
-    prefetch_tensormap(&tmap_a);
-    prefetch_tensormap(&tmap_b1);
-    if (kFused) prefetch_tensormap(&tmap_b2);
-    prefetch_tensormap(&tmap_y);
-    for (int s = 0; s < kStages; ++s) {
-      mbar_init(full_bar(s), 1);
-      mbar_init(empty_bar(s), 1);
+  if (warp == 0) {
+    if (lane == 0) {
+      prefetch_tensormap(&tmap_a);
+      prefetch_tensormap(&tmap_b1);
+      if (kFused) prefetch_tensormap(&tmap_b2);
+      prefetch_tensormap(&tmap_y);
+      for (int s = 0; s < kStages; ++s) {
+        mbar_init(full_bar(s), 1);
+        mbar_init(empty_bar(s), 1);
+      }
+      for (int a = 0; a < 2; ++a) {
+        mbar_init(acc_full_bar(a), 1);
+        mbar_init(acc_empty_bar(a), kEpiWarps * kCtaGroup);
+      }
+      fence_mbar_init();
+      fence_proxy_async_all();
     }
-    for (int a = 0; a < 2; ++a) {
-      mbar_init(acc_full_bar(a), 1);
-      mbar_init(acc_empty_bar(a), kEpiWarps * kCtaGroup);
+    if constexpr (kCtaGroup == 1 && kFused) {
+      if (lane == 0) {
+        // The producer needs only the barriers it has just initialised: fill the ring before
+        // the CTA-wide setup barrier so TMEM allocation overlaps the first loads' latency.
+        if (p.early_issue && group_id < total_tiles) {
+          pdl_wait_prior_grid();
+          int tm, tn;
+          decode_tile(p, group_id, tm, tn);
+          for (; pre < kStages && pre < k_blocks; ++pre)
+            issue_loads(pre, pre, tm * BM, tn * kOutCols);  // fresh ring: nothing to wait for
+        }
+      }
     }
-    fence_mbar_init();
   }
   if (warp == 1) tmem_alloc<kCtaGroup>(tmem_slot, kTmemCols);
   tcgen05_fence_before();
@@ -134,42 +191,16 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
 
   if (warp == 0 && lane == 0) {
     // ================================================================ TMA producer
-    int s = 0;
-    uint32_t ph = 0;
+    int s = (pre == kStages) ? 0 : pre;
+    uint32_t ph = (pre == kStages) ? 1u : 0u;
     for (int t = group_id; t < total_tiles; t += num_groups) {
       int tm, tn;
       decode_tile(p, t, tm, tn);
       const int m_base = (tm * kCtaGroup + (int)rank) * BM;
       const int n_base = tn * kOutCols;
-      for (int kb = 0; kb < k_blocks; ++kb) {
+      for (int kb = (t == group_id) ? pre : 0; kb < k_blocks; ++kb) {
         mbar_wait(empty_bar(s), ph ^ 1u);
-        if (rank == 0) mbar_arrive_expect_tx(full_bar(s), Cfg::kStageBytes * kCtaGroup);
-        const int k0 = kb * BK;
-        const uint32_t sa = smem_a(s), sb = smem_b(s), fb = full_bar(s);
-        if constexpr (kCtaGroup == 1) {
-          tma_load_2d(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
-          if constexpr (kFused) {
-            tma_load_2d(sb, &tmap_b1, fb, n_base, k0, kEvictNormal);
-            tma_load_2d(sb + 8192, &tmap_b1, fb, n_base + 64, k0, kEvictNormal);
-            tma_load_2d(sb + 16384, &tmap_b2, fb, n_base, k0, kEvictNormal);
-            tma_load_2d(sb + 24576, &tmap_b2, fb, n_base + 64, k0, kEvictNormal);
-          } else {
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-              tma_load_2d(sb + j * 8192, &tmap_b1, fb, n_base + j * 64, k0, kEvictNormal);
-          }
-        } else {
-          tma_load_2d_pair(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
-          if constexpr (kFused) {
-            const CUtensorMap* tb = (rank == 0) ? &tmap_b1 : &tmap_b2;
-            tma_load_2d_pair(sb, tb, fb, n_base, k0, kEvictNormal);
-            tma_load_2d_pair(sb + 8192, tb, fb, n_base + 64, k0, kEvictNormal);
-          } else {
-            const int nb = n_base + (int)rank * 128;
-            tma_load_2d_pair(sb, &tmap_b1, fb, nb, k0, kEvictNormal);
-            tma_load_2d_pair(sb + 8192, &tmap_b1, fb, nb + 64, k0, kEvictNormal);
-          }
-        }
+        issue_loads(s, kb, m_base, n_base);
         if (++s == kStages) { s = 0; ph ^= 1u; }
       }
     }
@@ -233,7 +264,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           if constexpr (kFused) {
             uint32_t g[32], u[32];
             tmem_ld_32x32b_x32(tacc + h * 64 + c * 32, g);
-            tmem_ld_32x32b_x32(tacc + 128 + h * 64 + c * 32, u);
+            tmem_ld_32x32b_x32(tacc + kBN + h * 64 + c * 32, u);
             tmem_ld_wait();
 #pragma unroll
             for (int j = 0; j < 16; ++j) {

@@ -40,11 +40,12 @@ enum FusedVariant {
   kFused1Cta = 0,     // 128x128 (Gate|Up) tile per CTA
   kFused2Cta = 1,     // 256x128 tile per CTA pair, cta_group::2
   kFusedSmallM = 2,   // swap-AB, split-K over a cluster, for M <= 128
-  kNumFused = 3
+  kFused1CtaN64 = 3,  // 128x64 (Gate|Up) tile per CTA: twice the tiles when N/128 < #SMs
+  kNumFused = 4
 };
 enum UnfusedVariant { kUnfused1Cta = 0, kUnfused2Cta = 1, kNumUnfused = 2 };
 const char* const kFusedNames[kNumFused] = {"fused_1cta_128x128", "fused_2cta_256x128",
-                                            "fused_smallm_swapab_splitk"};
+                                            "fused_smallm_swapab_splitk", "fused_1cta_128x64"};
 const char* const kUnfusedNames[kNumUnfused] = {"unfused_1cta_gemm128x256+silu_mul",
                                                 "unfused_2cta_gemm256x256+silu_mul"};
 
@@ -60,13 +61,18 @@ int select_fused(int64_t M, int64_t N, int64_t K) {
   if (forced >= 0 && forced < kNumFused) {
     if (forced != kFusedSmallM || M <= swiglu::kSmallMMax) return forced;
   }
-  if (M <= 64) return kFusedSmallM;
-  if (M <= 128) {
-    // HBM-bound either way; the 1-CTA kernel has one CTA per 128-column tile, so with fewer
-    // tiles than ~3/4 of the 148 SMs the split-K kernel (all SMs streaming) wins.
-    const int64_t n_tiles = (N + 127) / 128;
-    return (n_tiles * 4 <= 148 * 3) ? kFusedSmallM : kFused1Cta;
-  }
+  // Measured (profiles/r01_variant_sweep.md).  All of M <= 128 is HBM-bound; what matters is
+  // how many SMs stream weights and what the reduction costs:
+  //  * M <= 32: swap-AB split-K kernel (cluster DSMEM reduction is cheap for few rows);
+  //  * 32 < M <= 128: if N/128 tiles cannot fill ~3/4 of the 148 SMs, 64-column tiles (twice
+  //    the CTAs, no reduction); otherwise the split-K kernel up to M = 64 and the 128x128
+  //    1-CTA kernel above it;
+  //  * M > 128: the 2-CTA pair kernel.
+  const int64_t n_tiles = (N + 127) / 128;
+  const bool few_tiles = n_tiles * 4 <= 148 * 3;
+  if (M <= 32) return kFusedSmallM;
+  if (M <= 64) return few_tiles ? kFused1CtaN64 : kFusedSmallM;
+  if (M <= 128) return few_tiles ? kFused1CtaN64 : kFused1Cta;
   return kFused2Cta;
 }
 int select_unfused(int64_t M, int64_t N, int64_t K) {
@@ -155,6 +161,9 @@ int get_device_state(DeviceState** out) {
     CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true>,
                                   cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   GemmCfg<1>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true, 64>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  GemmCfg<1, 128>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, false>,
                                   cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   GemmCfg<1>::kSmemBytes));
@@ -210,7 +219,7 @@ bool pdl_enabled() {
 }
 
 // ------------------------------------------------------------------ launches
-template <int kCtaGroup, bool kFused>
+template <int kCtaGroup, bool kFused, int kBN = 128>
 int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void* B2, void* Yout,
                 int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
   using namespace swiglu;
@@ -220,10 +229,11 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   if ((rc = make_tmap(&tb1, B1, N, K, 64, 64))) return rc;
   if ((rc = make_tmap(&tb2, kFused ? B2 : B1, N, K, 64, 64))) return rc;
   if ((rc = make_tmap(&ty, Yout, N, M, 64, 128))) return rc;
+  using Cfg = GemmCfg<kCtaGroup, kFused ? 2 * kBN : 256>;
   GemmParams p;
   p.M = (int)M; p.N = (int)N; p.K = (int)K;
   const int rows_per_tile = BM * kCtaGroup;
-  const int out_cols = kFused ? 128 : 256;
+  const int out_cols = kFused ? kBN : 256;
   p.m_tiles = (int)((M + rows_per_tile - 1) / rows_per_tile);
   p.n_tiles = (int)((N + out_cols - 1) / out_cols);
   // L2 raster group: keep the slab of A the running CTAs share at <= 32 MiB
@@ -236,12 +246,14 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   const int64_t tiles = (int64_t)p.m_tiles * p.n_tiles;
   int groups = d.sm_count / kCtaGroup;
   if (tiles < groups) groups = (int)tiles;
+  // one tile per CTA (a short, HBM-bound call): fill the TMA ring before the setup barrier
+  p.early_issue = (kCtaGroup == 1 && kFused && tiles <= groups && !env_int("SWIGLU_NO_EARLY", 0));
 
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof cfg);
   cfg.gridDim = dim3((unsigned)(groups * kCtaGroup));
   cfg.blockDim = dim3(kGemmThreads);
-  cfg.dynamicSmemBytes = GemmCfg<kCtaGroup>::kSmemBytes;
+  cfg.dynamicSmemBytes = Cfg::kSmemBytes;
   cfg.stream = stream;
   cudaLaunchAttribute attrs[2];
   int na = 0;
@@ -259,15 +271,29 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   }
   cfg.attrs = attrs;
   cfg.numAttrs = na;
-  CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_swiglu_kernel<kCtaGroup, kFused>, ta, tb1, tb2, ty, p));
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_swiglu_kernel<kCtaGroup, kFused, kBN>, ta, tb1, tb2, ty,
+                              p));
   return SWIGLU_OK;
 }
 
-// Split-K factor of the small-M kernel: as many CTAs as can be co-resident, at most 8 per
-// cluster (portable cluster size), at least one k-block per CTA.
-int smallm_ksplit(int sm_count, int ctas_per_sm, int64_t n_tiles, int64_t k_blocks) {
+// Split-K factor of the small-M kernel (cluster size S), fitted to the measured sweep in
+// profiles/r01_smallm_ksplit_sweep.md:
+//  * at least as many 128-column tiles as SMs: no split (S = 1) -- except MP = 64, whose ring
+//    is only two stages deep, where two co-resident half-K CTAs per SM keep more bytes in flight;
+//  * fewer tiles than SMs: fill the co-resident CTA slots, but never more than 4 CTAs per
+//    cluster (clusters of 5-8 do not all fit at once and run in a second wave) and never fewer
+//    than 4 k-blocks per CTA (the cluster barrier + DSMEM reduction cost grows with S).
+int smallm_ksplit(int sm_count, int ctas_per_sm, int mp, int64_t n_tiles, int64_t k_blocks) {
   const int forced = env_int("SWIGLU_KSPLIT", 0);
-  int64_t s = ((int64_t)ctas_per_sm * sm_count) / n_tiles;
+  const int64_t slots = (int64_t)ctas_per_sm * sm_count;
+  int64_t s;
+  if (n_tiles >= sm_count) {
+    s = (mp == 64 && 2 * n_tiles <= slots) ? 2 : 1;
+  } else {
+    s = slots / n_tiles;
+    if (s > 4) s = 4;
+    while (s > 1 && k_blocks / s < 4) --s;
+  }
   if (forced > 0) s = forced;
   if (s > 8) s = 8;
   if (s > k_blocks) s = k_blocks;
@@ -287,7 +313,7 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   const int64_t n_tiles = (N + 127) / 128, k_blocks = (K + BK - 1) / BK;
   SmallParams p;
   p.M = (int)M; p.N = (int)N; p.K = (int)K;
-  p.ksplit = smallm_ksplit(d.sm_count, SmallCfg<MP>::kCtasPerSm, n_tiles, k_blocks);
+  p.ksplit = smallm_ksplit(d.sm_count, SmallCfg<MP>::kCtasPerSm, MP, n_tiles, k_blocks);
   p.ldy = N;
   // L2 prefetch ahead of the grid dependency: at most ~32 MiB over the whole grid
   const int64_t grid = n_tiles * p.ksplit;
@@ -407,6 +433,7 @@ int run_fused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
     case kFused1Cta: return launch_gemm<1, true>(*d, A, W1, W2, Y, M, N, K, stream);
     case kFused2Cta: return launch_gemm<2, true>(*d, A, W1, W2, Y, M, N, K, stream);
     case kFusedSmallM: return launch_smallm(*d, A, W1, W2, Y, M, N, K, stream);
+    case kFused1CtaN64: return launch_gemm<1, true, 64>(*d, A, W1, W2, Y, M, N, K, stream);
   }
   return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
 }

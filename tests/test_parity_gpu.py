@@ -68,7 +68,7 @@ ODD_SHAPES = [
     (1, 128, 64), (7, 136, 72), (16, 384, 896), (127, 128, 64), (128, 4864, 896),
     (129, 264, 200), (300, 1160, 328), (513, 392, 1096),
 ]
-VARIANTS = [("fused", 0), ("fused", 1), ("unfused", 0), ("unfused", 1)]
+VARIANTS = [("fused", 0), ("fused", 1), ("fused", 3), ("unfused", 0), ("unfused", 1)]
 
 
 @pytest.mark.parametrize("kind,variant", VARIANTS)
