@@ -54,7 +54,27 @@ struct GemmParams {
   int n_tiles;   // ceil(N / (fused ? 128 : 256))
   int group_m;   // m-tiles per L2 raster group
   int early_issue;      // 1: fill the ring before the CTA-wide setup barrier (small grids)
+#ifdef SWIGLU_TRACE
+  unsigned long long* trace;  // [grid][kGemmTraceStride] globaltimer stamps (debug builds only)
+#endif
 };
+
+// Debug-build timeline stamps (compiled out unless -DSWIGLU_TRACE): slot i of this CTA.
+constexpr int kGemmTraceStride = 8 + 8 * 32;
+#ifdef SWIGLU_TRACE
+#define SWIGLU_TRACE_POINT(i)                                                         \
+  do {                                                                                \
+    if (p.trace) p.trace[(size_t)blockIdx.x * 16 + (i)] = globaltimer_ns();           \
+  } while (0)
+#define SWIGLU_GEMM_TRACE(i)                                                          \
+  do {                                                                                \
+    if (p.trace && (i) < kGemmTraceStride)                                            \
+      p.trace[(size_t)blockIdx.x * kGemmTraceStride + (i)] = globaltimer_ns();        \
+  } while (0)
+#else
+#define SWIGLU_TRACE_POINT(i) do { } while (0)
+#define SWIGLU_GEMM_TRACE(i) do { } while (0)
+#endif
 
 // Tile order: groups of `group_m` row-tiles x all column-tiles, row-tile fastest inside a
 // group, so the CTAs running at one time share a slab of A that stays in L2 and stream W.
@@ -146,6 +166,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   int pre = 0;  // k-blocks of this CTA's first tile issued before the setup barrier
 
   // ------------------------------------------------------------------ one-time setup
+  if (threadIdx.x == 0) SWIGLU_GEMM_TRACE(0);
   if (warp == 0) {
     if (lane == 0) {
       prefetch_tensormap(&tmap_a);
@@ -188,6 +209,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   // unfused path, the Gate/Up it wrote) must be complete before we touch global memory.
   pdl_wait_prior_grid();
   pdl_launch_dependents();  // the next kernel may start its own prologue as SMs free up
+  if (threadIdx.x == 0) SWIGLU_GEMM_TRACE(1);
 
   if (warp == 0 && lane == 0) {
     // ================================================================ TMA producer
@@ -215,10 +237,12 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1u;
       mbar_wait(acc_empty_bar(as), aph ^ 1u);  // epilogue has drained this TMEM stage
+      SWIGLU_GEMM_TRACE(8 + it * 8 + 0);
       tcgen05_fence_after();
       const uint32_t d_tmem = tmem_base + as * UMMA_N;
       for (int kb = 0; kb < k_blocks; ++kb) {
         mbar_wait(full_bar(s), ph);
+        if (kb == 0) SWIGLU_GEMM_TRACE(8 + it * 8 + 1);
         tcgen05_fence_after();
         const uint32_t sa = smem_a(s), sb = smem_b(s);
 #pragma unroll
@@ -233,6 +257,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
         if (++s == kStages) { s = 0; ph ^= 1u; }
       }
       umma_commit<kCtaGroup>(acc_full_bar(as));  // accumulator complete -> epilogue
+      SWIGLU_GEMM_TRACE(8 + it * 8 + 2);
     }
   } else if (warp >= 2) {
     // ================================================================ epilogue
@@ -250,6 +275,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1u;
       mbar_wait(acc_full_bar(as), aph);
+      if (issuer) SWIGLU_GEMM_TRACE(8 + it * 8 + 3);
       tcgen05_fence_after();
       const uint32_t tacc = tmem_base + ((q * 32u) << 16) + as * UMMA_N;
 #pragma unroll 1
@@ -305,6 +331,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           tma_store_commit();
         }
       }
+      if (issuer) SWIGLU_GEMM_TRACE(8 + it * 8 + 4);
     }
     if (issuer) tma_store_wait_all<0>();
   }
@@ -317,6 +344,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     tcgen05_fence_after();
     tmem_dealloc<kCtaGroup>(tmem_base, kTmemCols);
   }
+  if (threadIdx.x == 0) SWIGLU_GEMM_TRACE(2);
 }
 
 // ---------------------------------------------------------------------------------------

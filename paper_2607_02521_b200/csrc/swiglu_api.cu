@@ -35,6 +35,10 @@ int fail_cuda(cudaError_t e, const char* what) {
     if (_e != cudaSuccess) return fail_cuda(_e, #expr);  \
   } while (0)
 
+#ifdef SWIGLU_TRACE
+unsigned long long* g_trace = nullptr;  // debug builds: device buffer for globaltimer stamps
+#endif
+
 // ------------------------------------------------------------------ variant tables
 enum FusedVariant {
   kFused1Cta = 0,     // 128x128 (Gate|Up) tile per CTA
@@ -209,10 +213,6 @@ int make_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
   return SWIGLU_OK;
 }
 
-#ifdef SWIGLU_TRACE
-unsigned long long* g_trace = nullptr;  // debug builds: device buffer for globaltimer stamps
-#endif
-
 bool pdl_enabled() {
   static const bool on = env_int("SWIGLU_NO_PDL", 0) == 0;
   return on;
@@ -248,6 +248,9 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   if (tiles < groups) groups = (int)tiles;
   // one tile per CTA (a short, HBM-bound call): fill the TMA ring before the setup barrier
   p.early_issue = (kCtaGroup == 1 && kFused && tiles <= groups && !env_int("SWIGLU_NO_EARLY", 0));
+#ifdef SWIGLU_TRACE
+  p.trace = g_trace;
+#endif
 
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof cfg);
