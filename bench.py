@@ -302,6 +302,22 @@ def measure_points(wl, peaks, do_check=True, Ms=None):
              "roofline_frac_sustained": round(t_sus / t, 4),
              "unfused_us": round(u["us_median"], 2),
              "speedup_vs_unfused": round(u["us_median"] / f["us_median"], 3)}
+        # Fusion-efficiency ablation (Table 6): the standalone
+        # elementwise stage gives BW_eff; eta = saved time / (4*M*N*2 bytes / BW_eff).
+        import torch
+        gu = torch.empty((2, M, wl.N), dtype=torch.bfloat16, device="cuda").normal_()
+        lib = B.load()
+
+        def ew(a, w1, w2, y, m, n, k, stream, _g=gu[0].data_ptr(), _u=gu[1].data_ptr()):
+            return lib.swiglu_silu_mul(_g, _u, y, m * n, stream)
+        e = time_point(wl, ew, M)
+        bw_eff = 6.0 * M * wl.N / (e["us_median"] * 1e-6)            # bytes/s: read G, U, write Y
+        saved = (u["us_median"] - f["us_median"]) * 1e-6
+        p["elementwise_us"] = round(e["us_median"], 2)
+        p["swiglu_share_of_unfused"] = round(e["us_median"] / u["us_median"], 4)
+        p["bw_eff_gbs"] = round(bw_eff / 1e9, 1)
+        p["fusion_efficiency"] = round(saved / (8.0 * M * wl.N / bw_eff), 3)
+        del gu
         if do_check:
             p["parity"] = check_point(wl, M)
         pts.append(p)
@@ -533,8 +549,9 @@ def run_all(args):
     json.dump({"peaks": peaks, "peak_source": peak_src, "clocks": clocks, "points": pts},
               open(os.path.join(ROOT, "gpurun_out", "results.json"), "w"), indent=1)
     hdr = ("| workload | M | variant | us | TFLOP/s | GB/s | bound | % of measured roofline | "
-           "% of nominal | unfused us | speed-up | mismatches fused / unfused (checked) |")
-    lines = [hdr, "|" + "---|" * 12]
+           "% of nominal | unfused us | speed-up | elementwise us (share of unfused) | "
+           "fusion eff. | mismatches fused / unfused (checked) |")
+    lines = [hdr, "|" + "---|" * 14]
     for p in pts:
         par = p.get("parity")
         ptxt = (f"{par['fused']['mismatches']} / {par['unfused']['mismatches']} ({par['fused']['checked']})"
@@ -542,7 +559,8 @@ def run_all(args):
         lines.append(f"| {p['workload']} | {p['M']} | {p['variant']} | {p['us']} | {p['tflops']} | "
                      f"{p['gbs']} | {p['bound']} | {100 * p['roofline_frac']:.1f} | "
                      f"{100 * p['roofline_frac_nominal']:.1f} | {p['unfused_us']} | "
-                     f"{p['speedup_vs_unfused']} | {ptxt} |")
+                     f"{p['speedup_vs_unfused']} | {p['elementwise_us']} "
+                     f"({100 * p['swiglu_share_of_unfused']:.0f} %) | {p['fusion_efficiency']} | {ptxt} |")
     md = "\n".join(lines)
     open(os.path.join(ROOT, "gpurun_out", "results.md"), "w").write(md + "\n")
     print(md)

@@ -94,6 +94,15 @@ int swiglu_mlp_unfused_ex(const void* A, const void* W1, const void* W2, void* Y
                           int64_t N, int64_t K, void* workspace, size_t workspace_bytes,
                           int variant, void* stream);
 
+/*
+ * The elementwise stage of the unfused path on its own (read Gate,
+ * read Up, write Y; the "standalone SwiGLU" the paper profiles for its effective bandwidth,
+ * line 321): Y[i] = bf16(SiLU(float(G[i])) * float(U[i])) for i < elems.  G, U, Y: device
+ * pointers to bf16, 16-byte aligned; Y may alias G or U exactly (in place) but not partially;
+ * elems must be a multiple of 8.  Asynchronous on `stream`.
+ */
+int swiglu_silu_mul(const void* G, const void* U, void* Y, int64_t elems, void* stream);
+
 /* Bytes of workspace the given variant (-1 = automatic) needs; 0 if none or bad arguments.
  * `unfused` != 0 asks about swiglu_mlp_unfused. */
 size_t swiglu_workspace_bytes(int64_t M, int64_t N, int64_t K, int unfused, int variant);

@@ -25,7 +25,7 @@ SWIGLU_ERR_WORKSPACE = 7
 SWIGLU_ERR_CUDA = 8
 
 EXPORTS = (
-    "swiglu_mlp", "swiglu_mlp_unfused", "swiglu_mlp_ex", "swiglu_mlp_unfused_ex",
+    "swiglu_mlp", "swiglu_mlp_unfused", "swiglu_mlp_ex", "swiglu_mlp_unfused_ex", "swiglu_silu_mul",
     "swiglu_workspace_bytes", "swiglu_num_variants", "swiglu_variant_name",
     "swiglu_selected_variant", "swiglu_launches_per_call", "swiglu_validate",
     "swiglu_mlp_host", "swiglu_last_error", "swiglu_status_string", "swiglu_version",
@@ -65,6 +65,7 @@ def load():
     lib.swiglu_launches_per_call.argtypes, lib.swiglu_launches_per_call.restype = [i64, i64, i64, ci, ci], ci
     lib.swiglu_validate.argtypes, lib.swiglu_validate.restype = [p, p, p, p, i64, i64, i64], ci
     lib.swiglu_mlp_host.argtypes, lib.swiglu_mlp_host.restype = [p, p, p, p, i64, i64, i64, ci, p], ci
+    lib.swiglu_silu_mul.argtypes, lib.swiglu_silu_mul.restype = [p, p, p, i64, p], ci
     lib.swiglu_last_error.argtypes, lib.swiglu_last_error.restype = [], ctypes.c_char_p
     lib.swiglu_status_string.argtypes, lib.swiglu_status_string.restype = [ci], ctypes.c_char_p
     lib.swiglu_version.argtypes, lib.swiglu_version.restype = [], ctypes.c_char_p
@@ -149,6 +150,13 @@ def swiglu_mlp_unfused_ex(A, W1, W2, Y, M=None, N=None, K=None, workspace=None,
     _check(load().swiglu_mlp_unfused_ex(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), m, n, k,
                                         _ptr(workspace), int(workspace_bytes), int(variant),
                                         _stream(stream)))
+
+
+def swiglu_silu_mul(G, U, Y, elems=None, stream=None) -> None:
+    """Elementwise stage alone: Y = bf16(SiLU(G) * U) over `elems` bf16 values (device)."""
+    if elems is None:
+        elems = int(G.numel())
+    _check(load().swiglu_silu_mul(_ptr(G), _ptr(U), _ptr(Y), int(elems), _stream(stream)))
 
 
 def swiglu_mlp_host(A_host, W1_host, W2_host, Y_host, M, N, K, unfused=False, stream=None) -> None:

@@ -53,6 +53,8 @@ struct GemmParams {
   int m_tiles;   // ceil(M / (128*kCtaGroup))
   int n_tiles;   // ceil(N / (fused ? 128 : 256))
   int group_m;   // m-tiles per L2 raster group
+  int wide_tiles;   // tiles [0, wide_tiles) are full width; the rest are 64-column half tiles
+  int total_tiles;  // wide_tiles + 2 * (m_tiles*n_tiles - wide_tiles)
   int early_issue;      // 1: fill the ring before the CTA-wide setup barrier (small grids)
 #ifdef SWIGLU_TRACE
   unsigned long long* trace;  // [grid][kGemmTraceStride] globaltimer stamps (debug builds only)
@@ -96,6 +98,26 @@ __device__ __forceinline__ float silu_mul(float g, float u) {
   return (g * u) * r;
 }
 
+// Tile t of the schedule -> (row tile, first output column, width in output columns).
+// The last partial wave of a fused 128-column schedule may be cut into 64-column half tiles
+// (two consecutive schedule slots per wide tile), so that it occupies all SMs for half a
+// tile time instead of half the SMs for a whole one (a1: wave quantisation).
+template <int kOutCols>
+__device__ __forceinline__ void decode_tile_w(const GemmParams& p, int t, int& tm, int& n_base,
+                                              int& w) {
+  int tn;
+  if (t < p.wide_tiles) {
+    decode_tile(p, t, tm, tn);
+    n_base = tn * kOutCols;
+    w = kOutCols;
+  } else {
+    const int j = t - p.wide_tiles;
+    decode_tile(p, p.wide_tiles + (j >> 1), tm, tn);
+    n_base = tn * kOutCols + (j & 1) * 64;
+    w = 64;
+  }
+}
+
 template <int kCtaGroup, bool kFused, int kBN = 128>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
@@ -127,24 +149,31 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   const uint32_t rank = (kCtaGroup == 2) ? cluster_ctarank() : 0u;
   const int num_groups = gridDim.x / kCtaGroup;  // CTAs (or CTA pairs) sharing the tile list
   const int group_id = blockIdx.x / kCtaGroup;
-  const int total_tiles = p.m_tiles * p.n_tiles;
+  const int total_tiles = p.total_tiles;
   const int k_blocks = (p.K + BK - 1) / BK;
 
   // One k-block of A and B into ring slot s (no waiting here: the caller owns the ring state).
-  auto issue_loads = [&](int s, int kb, int m_base, int n_base) {
-    if (rank == 0) mbar_arrive_expect_tx(full_bar(s), Cfg::kStageBytes * kCtaGroup);
+  // w = output columns of the tile (kOutCols, or 64 for a half tile of the last wave).
+  auto issue_loads = [&](int s, int kb, int m_base, int n_base, int w) {
+    const bool half = kFused && kBN == 128 && w == 64;
+    if (rank == 0) {
+      const uint32_t b_bytes = half ? Cfg::kBBytes / 2 : Cfg::kBBytes;
+      mbar_arrive_expect_tx(full_bar(s), (Cfg::kABytes + b_bytes) * kCtaGroup);
+    }
     const int k0 = kb * BK;
     const uint32_t sa = smem_a(s), sb = smem_b(s), fb = full_bar(s);
     if constexpr (kCtaGroup == 1) {
       tma_load_2d(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
-      if constexpr (kFused && kBN == 64) {
-        tma_load_2d(sb, &tmap_b1, fb, n_base, k0, kEvictNormal);
-        tma_load_2d(sb + 8192, &tmap_b2, fb, n_base, k0, kEvictNormal);
-      } else if constexpr (kFused) {
-        tma_load_2d(sb, &tmap_b1, fb, n_base, k0, kEvictNormal);
-        tma_load_2d(sb + 8192, &tmap_b1, fb, n_base + 64, k0, kEvictNormal);
-        tma_load_2d(sb + 16384, &tmap_b2, fb, n_base, k0, kEvictNormal);
-        tma_load_2d(sb + 24576, &tmap_b2, fb, n_base + 64, k0, kEvictNormal);
+      if constexpr (kFused) {
+        if (kBN == 64 || half) {  // W1 atom | W2 atom
+          tma_load_2d(sb, &tmap_b1, fb, n_base, k0, kEvictNormal);
+          tma_load_2d(sb + 8192, &tmap_b2, fb, n_base, k0, kEvictNormal);
+        } else {                  // W1 atoms 0,1 | W2 atoms 0,1
+          tma_load_2d(sb, &tmap_b1, fb, n_base, k0, kEvictNormal);
+          tma_load_2d(sb + 8192, &tmap_b1, fb, n_base + 64, k0, kEvictNormal);
+          tma_load_2d(sb + 16384, &tmap_b2, fb, n_base, k0, kEvictNormal);
+          tma_load_2d(sb + 24576, &tmap_b2, fb, n_base + 64, k0, kEvictNormal);
+        }
       } else {
 #pragma unroll
         for (int j = 0; j < 4; ++j)
@@ -155,7 +184,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       if constexpr (kFused) {
         const CUtensorMap* tb = (rank == 0) ? &tmap_b1 : &tmap_b2;
         tma_load_2d_pair(sb, tb, fb, n_base, k0, kEvictNormal);
-        tma_load_2d_pair(sb + 8192, tb, fb, n_base + 64, k0, kEvictNormal);
+        if (!half) tma_load_2d_pair(sb + 8192, tb, fb, n_base + 64, k0, kEvictNormal);
       } else {
         const int nb = n_base + (int)rank * 128;
         tma_load_2d_pair(sb, &tmap_b1, fb, nb, k0, kEvictNormal);
@@ -190,10 +219,10 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
         // the CTA-wide setup barrier so TMEM allocation overlaps the first loads' latency.
         if (p.early_issue && group_id < total_tiles) {
           pdl_wait_prior_grid();
-          int tm, tn;
-          decode_tile(p, group_id, tm, tn);
+          int tm, n_base, w;
+          decode_tile_w<kOutCols>(p, group_id, tm, n_base, w);
           for (; pre < kStages && pre < k_blocks; ++pre)
-            issue_loads(pre, pre, tm * BM, tn * kOutCols);  // fresh ring: nothing to wait for
+            issue_loads(pre, pre, tm * BM, n_base, w);  // fresh ring: nothing to wait for
         }
       }
     }
@@ -216,20 +245,20 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     int s = (pre == kStages) ? 0 : pre;
     uint32_t ph = (pre == kStages) ? 1u : 0u;
     for (int t = group_id; t < total_tiles; t += num_groups) {
-      int tm, tn;
-      decode_tile(p, t, tm, tn);
+      int tm, n_base, w;
+      decode_tile_w<kOutCols>(p, t, tm, n_base, w);
       const int m_base = (tm * kCtaGroup + (int)rank) * BM;
-      const int n_base = tn * kOutCols;
       for (int kb = (t == group_id) ? pre : 0; kb < k_blocks; ++kb) {
         mbar_wait(empty_bar(s), ph ^ 1u);
-        issue_loads(s, kb, m_base, n_base);
+        issue_loads(s, kb, m_base, n_base, w);
         if (++s == kStages) { s = 0; ph ^= 1u; }
       }
     }
   } else if (warp == 1 && lane == 0 && rank == 0) {
     // ================================================================ MMA issuer
-    constexpr uint32_t idesc = idesc_bf16_f32(BM * kCtaGroup, UMMA_N, /*a_mn=*/false,
-                                              /*b_mn=*/true);
+    constexpr uint32_t idesc_full = idesc_bf16_f32(BM * kCtaGroup, UMMA_N, /*a_mn=*/false,
+                                                   /*b_mn=*/true);
+    constexpr uint32_t idesc_half = idesc_bf16_f32(BM * kCtaGroup, 128, false, true);
     int s = 0;
     uint32_t ph = 0;
     int it = 0;
@@ -240,6 +269,8 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       SWIGLU_GEMM_TRACE(8 + it * 8 + 0);
       tcgen05_fence_after();
       const uint32_t d_tmem = tmem_base + as * UMMA_N;
+      // half tiles of the last wave (Gate 64 | Up 64) use an N = 128 instruction
+      const uint32_t idesc = (kFused && kBN == 128 && t >= p.wide_tiles) ? idesc_half : idesc_full;
       for (int kb = 0; kb < k_blocks; ++kb) {
         mbar_wait(full_bar(s), ph);
         if (kb == 0) SWIGLU_GEMM_TRACE(8 + it * 8 + 1);
@@ -268,10 +299,10 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     int it = 0;
     uint32_t chunk_ctr = 0;
     for (int t = group_id; t < total_tiles; t += num_groups, ++it) {
-      int tm, tn;
-      decode_tile(p, t, tm, tn);
+      int tm, n_base, w;
+      decode_tile_w<kOutCols>(p, t, tm, n_base, w);
       const int m_base = (tm * kCtaGroup + (int)rank) * BM;
-      const int n_base = tn * kOutCols;
+      const int chunks = kFused ? w / 64 : kChunks;  // 64-column chunks in this tile
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1u;
       mbar_wait(acc_full_bar(as), aph);
@@ -279,7 +310,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       tcgen05_fence_after();
       const uint32_t tacc = tmem_base + ((q * 32u) << 16) + as * UMMA_N;
 #pragma unroll 1
-      for (int h = 0; h < kChunks; ++h, ++chunk_ctr) {
+      for (int h = 0; h < chunks; ++h, ++chunk_ctr) {
         const uint32_t obuf = smem_out + (chunk_ctr & 1u) * kOutBufBytes;
         // the TMA store that last read this buffer (2 chunks ago) must have finished reading
         if (issuer) tma_store_wait_read<1>();
@@ -290,7 +321,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           if constexpr (kFused) {
             uint32_t g[32], u[32];
             tmem_ld_32x32b_x32(tacc + h * 64 + c * 32, g);
-            tmem_ld_32x32b_x32(tacc + kBN + h * 64 + c * 32, u);
+            tmem_ld_32x32b_x32(tacc + w + h * 64 + c * 32, u);  // Up starts at column w
             tmem_ld_wait();
 #pragma unroll
             for (int j = 0; j < 16; ++j) {
@@ -307,7 +338,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
             for (int j = 0; j < 16; ++j)
               packed[j] = pack_bf16x2_rn(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
           }
-          if (h == kChunks - 1 && c == 1) {
+          if (h == chunks - 1 && c == 1) {
             // last TMEM read of this tile is done: hand the accumulator stage back to the MMA
             tcgen05_fence_before();
             __syncwarp();

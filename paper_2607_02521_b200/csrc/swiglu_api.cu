@@ -246,6 +246,17 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   const int64_t tiles = (int64_t)p.m_tiles * p.n_tiles;
   int groups = d.sm_count / kCtaGroup;
   if (tiles < groups) groups = (int)tiles;
+  // Last partial wave: if at most half of the CTA groups would get a tile, cut those tiles into
+  // 64-column halves so the wave takes half a tile time on all SMs (fused 128-column tiles only).
+  p.wide_tiles = (int)tiles;
+  p.total_tiles = (int)tiles;
+  if (kFused && kBN == 128 && tiles > groups && !env_int("SWIGLU_NO_TAIL_SPLIT", 0)) {
+    const int64_t rem = tiles % groups;
+    if (rem > 0 && 2 * rem <= groups) {
+      p.wide_tiles = (int)(tiles - rem);
+      p.total_tiles = (int)(tiles + rem);
+    }
+  }
   // one tile per CTA (a short, HBM-bound call): fill the TMA ring before the setup barrier
   p.early_issue = (kCtaGroup == 1 && kFused && tiles <= groups && !env_int("SWIGLU_NO_EARLY", 0));
 #ifdef SWIGLU_TRACE
@@ -502,6 +513,19 @@ int swiglu_mlp_unfused_ex(const void* A, const void* W1, const void* W2, void* Y
                           int variant, void* stream) {
   return run_unfused(A, W1, W2, Y, M, N, K, workspace, workspace_bytes, false, variant,
                      (cudaStream_t)stream);
+}
+
+int swiglu_silu_mul(const void* G, const void* U, void* Y, int64_t elems, void* stream) {
+  if (elems < 0) return fail(SWIGLU_ERR_BAD_SHAPE, "elems=%lld < 0", (long long)elems);
+  if (elems % 8) return fail(SWIGLU_ERR_UNSUPPORTED, "elems=%lld must be a multiple of 8", (long long)elems);
+  if (elems == 0) return SWIGLU_OK;
+  if (!G || !U || !Y) return fail(SWIGLU_ERR_NULL_POINTER, "G, U or Y is NULL");
+  if (((uintptr_t)G | (uintptr_t)U | (uintptr_t)Y) & 15u)
+    return fail(SWIGLU_ERR_MISALIGNED, "G, U and Y must be 16-byte aligned");
+  DeviceState* d;
+  int rc = get_device_state(&d);
+  if (rc) return rc;
+  return launch_silu_mul(*d, G, U, Y, elems, (cudaStream_t)stream);
 }
 
 size_t swiglu_workspace_bytes(int64_t M, int64_t N, int64_t K, int unfused, int variant) {

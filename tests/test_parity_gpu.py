@@ -101,6 +101,20 @@ def test_small_m_kernel_every_cluster_size(M, ksplit, monkeypatch):
     assert_parity(run("fused", 2, A, W1, W2), y_ref, ("smallm", M, ksplit))
 
 
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("M,N,K", [(2560, 1024, 128), (2560, 1032, 72), (2305, 1160, 64)])
+def test_last_wave_half_tiles(variant, M, N, K, monkeypatch):
+    """Shapes whose tile count leaves a last wave of <= half the CTA groups: those tiles run as
+    64-column half tiles (a1).  Same result with the split disabled."""
+    A, W1, W2 = inputs.make_case(M, N, K, seed=400 + N + K, std=0.05)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+    y_split = run("fused", variant, A, W1, W2)
+    assert_parity(y_split, y_ref, ("tail-split", variant, M, N, K))
+    monkeypatch.setenv("SWIGLU_NO_TAIL_SPLIT", "1")
+    y_plain = run("fused", variant, A, W1, W2)
+    assert_parity(y_plain, y_ref, ("no-split", variant, M, N, K))
+
+
 def test_small_m_variant_rejects_large_m():
     A, W1, W2 = inputs.make_case(129, 128, 64, seed=1)
     with pytest.raises(B.SwigluError) as e:
@@ -143,6 +157,26 @@ def test_baseline_full_sizes_sampled_rows(shape):
             rep = check.compare(host(dY[torch.from_numpy(rows).cuda()]), y_ref)
             assert rep.mismatches == 0, (shape, M, entry.__name__, rep)
             del dY
+
+
+def test_elementwise_stage_alone():
+    """swiglu_silu_mul against the oracle's own fp64 SiLU on bf16 Gate/Up values (including
+    the tails |g| up to 40 where SiLU -> g and SiLU -> 0-), ragged length (multiple of 8)."""
+    rng = np.random.Generator(np.random.Philox(key=77))
+    n = 8 * 12345
+    g = inputs.f32_to_bf16_bits((rng.standard_normal(n) * 4).astype(np.float32))
+    u = inputs.f32_to_bf16_bits(rng.standard_normal(n).astype(np.float32))
+    g[:8] = inputs.f64_to_bf16_bits_exact([0.0, 1.0, -1.0, 40.0, -40.0, 10.0, -10.0, 0.5])
+    dG, dU = dev(g), dev(u)
+    dY = torch.full((n,), float("nan"), dtype=torch.bfloat16, device="cuda")
+    B.swiglu_silu_mul(dG, dU, dY)
+    torch.cuda.synchronize()
+    g64, u64 = inputs.bf16_bits_to_f64(g), inputs.bf16_bits_to_f64(u)
+    y_ref = np.array([oracle.silu(x) for x in g64]) * u64
+    assert_parity(host(dY), y_ref, "silu_mul")
+    with pytest.raises(B.SwigluError) as e:
+        B.swiglu_silu_mul(dG, dU, dY, elems=12)
+    assert e.value.status == B.SWIGLU_ERR_UNSUPPORTED
 
 
 def test_invariants_on_gpu():
