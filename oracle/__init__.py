@@ -8,6 +8,8 @@ The arithmetic lives in ``swiglu_oracle.c`` (plain C, fp64; PAPER.md lines 86-94
 this module only compiles that file with gcc and marshals numpy arrays into it.
 """
 from .oracle import (  # noqa: F401
+    ACTIVATIONS,
+    activation,
     build,
     max_threads,
     silu,

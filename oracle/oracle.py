@@ -45,6 +45,13 @@ def _load():
         lib.swiglu_oracle.restype = ctypes.c_int
         lib.swiglu_oracle_rows.argtypes = [p, p, p, p, p, i64, i64, i64, i64, ctypes.c_int]
         lib.swiglu_oracle_rows.restype = ctypes.c_int
+        lib.swiglu_oracle_act.argtypes = [p, p, p, p, i64, i64, i64, ctypes.c_int, ctypes.c_int]
+        lib.swiglu_oracle_act.restype = ctypes.c_int
+        lib.swiglu_oracle_rows_act.argtypes = [p, p, p, p, p, i64, i64, i64, i64, ctypes.c_int,
+                                               ctypes.c_int]
+        lib.swiglu_oracle_rows_act.restype = ctypes.c_int
+        lib.swiglu_oracle_activation.argtypes = [ctypes.c_int, ctypes.c_double]
+        lib.swiglu_oracle_activation.restype = ctypes.c_double
         lib.swiglu_oracle_silu.argtypes = [ctypes.c_double]
         lib.swiglu_oracle_silu.restype = ctypes.c_double
         lib.swiglu_oracle_max_threads.argtypes = []
@@ -75,8 +82,17 @@ def silu(x: float) -> float:
     return float(_load().swiglu_oracle_silu(float(x)))
 
 
-def swiglu_oracle(A_bits, W1_bits, W2_bits, nthreads: int = 0):
-    """y_ref[M,N] in fp64 from bf16 bit patterns A[M,K], W1[K,N], W2[K,N] (uint16).
+ACTIVATIONS = {"silu": 0, "gelu": 1, "gelu_tanh": 2, "relu": 3}
+
+
+def activation(act, x: float) -> float:
+    """The oracle's own fp64 gate activation (act: name or id), for the pins."""
+    return float(_load().swiglu_oracle_activation(int(ACTIVATIONS.get(act, act)), float(x)))
+
+
+def swiglu_oracle(A_bits, W1_bits, W2_bits, nthreads: int = 0, act=0):
+    """y_ref[M,N] in fp64 from bf16 bit patterns A[M,K], W1[K,N], W2[K,N] (uint16);
+    act = 0/"silu" (the paper's Eq. 3), "gelu", "gelu_tanh", "relu" (GeGLU / ReGLU).
 
     Returns (y_ref, threads_used)."""
     A_bits = np.ascontiguousarray(A_bits)
@@ -91,13 +107,14 @@ def swiglu_oracle(A_bits, W1_bits, W2_bits, nthreads: int = 0):
     W1 = _bits(W1_bits, (K, N), "W1")
     W2 = _bits(W2_bits, (K, N), "W2")
     Y = np.empty((M, N), dtype=np.float64)
-    used = _load().swiglu_oracle(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), M, N, K, int(nthreads))
+    used = _load().swiglu_oracle_act(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), M, N, K,
+                                     int(ACTIVATIONS.get(act, act)), int(nthreads))
     if used < 0:
         raise RuntimeError("swiglu_oracle rejected its arguments")
     return Y, int(used)
 
 
-def swiglu_oracle_rows(A_bits, W1_bits, W2_bits, rows, nthreads: int = 0):
+def swiglu_oracle_rows(A_bits, W1_bits, W2_bits, rows, nthreads: int = 0, act=0):
     """Rows ``rows`` of y_ref only (full N columns each): [len(rows), N] fp64."""
     A_bits = np.ascontiguousarray(A_bits)
     W1_bits = np.ascontiguousarray(W1_bits)
@@ -110,8 +127,9 @@ def swiglu_oracle_rows(A_bits, W1_bits, W2_bits, rows, nthreads: int = 0):
     W2 = _bits(W2_bits, (K, N), "W2")
     r = np.ascontiguousarray(np.asarray(rows, dtype=np.int64))
     Y = np.empty((r.shape[0], N), dtype=np.float64)
-    used = _load().swiglu_oracle_rows(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), _ptr(r),
-                                      r.shape[0], M, N, K, int(nthreads))
+    used = _load().swiglu_oracle_rows_act(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), _ptr(r),
+                                          r.shape[0], M, N, K, int(ACTIVATIONS.get(act, act)),
+                                          int(nthreads))
     if used < 0:
         raise RuntimeError("swiglu_oracle_rows rejected its arguments")
     return Y, int(used)

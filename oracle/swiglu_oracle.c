@@ -60,10 +60,40 @@ double swiglu_oracle_silu(double x) {
   }
 }
 
+/*
+ * The other gated activations of the GLU family the paper names ("gated
+ * linear unit variants (GEGLU, SwiGLU, ReGLU)", Shazeer 2020; line 392 future-work item 4:
+ * "generalization to other gated activations (GeGLU, ReGLU)"): Y = act(Gate) (.) Up with
+ *   act 0  SiLU       x * sigma(x)                                   (Eq. 3, the paper's)
+ *   act 1  GELU       x * Phi(x) = 0.5 * x * erfc(-x / sqrt(2))      (GeGLU, exact form)
+ *   act 2  GELU-tanh  0.5 * x * (1 + tanh(sqrt(2/pi) * (x + 0.044715 x^3)))   (GeGLU, the
+ *          tanh approximation most frameworks ship; reading R17), evaluated as
+ *          x * sigma(2 * sqrt(2/pi) * (x + 0.044715 x^3)), the same function
+ *   act 3  ReLU       max(x, 0)                                      (ReGLU)
+ * GELU is written with erfc so that the negative tail keeps its relative accuracy.
+ */
+double swiglu_oracle_activation(int act, double x) {
+  switch (act) {
+    case 0: return swiglu_oracle_silu(x);
+    case 1: return 0.5 * x * erfc(-x / sqrt(2.0));
+    case 2: {
+      /* 0.5*(1 + tanh(u)) = sigma(2u) exactly; written through exp so that the negative tail
+       * does not cancel (1 + tanh(u) loses all its digits for u << 0).  DESIGN.md R17. */
+      const double c = sqrt(2.0 / acos(-1.0));
+      const double z = 2.0 * c * (x + 0.044715 * x * x * x);
+      if (z >= 0.0) return x / (1.0 + exp(-z));
+      const double e = exp(z);
+      return x * e / (1.0 + e);
+    }
+    case 3: return x > 0.0 ? x : 0.0;
+  }
+  return NAN;
+}
+
 /* One work unit: row m, columns [n0, n1).  gate/up are caller-provided scratch of PANEL. */
 static void unit(const uint16_t *A, const uint16_t *W1, const uint16_t *W2, double *Y,
                  int64_t N, int64_t K, int64_t m, int64_t n0, int64_t n1, double *gate,
-                 double *up) {
+                 double *up, int act) {
   const int64_t w = n1 - n0;
   for (int64_t j = 0; j < w; ++j) {
     gate[j] = 0.0;
@@ -79,7 +109,7 @@ static void unit(const uint16_t *A, const uint16_t *W1, const uint16_t *W2, doub
     }
   }
   for (int64_t j = 0; j < w; ++j) {
-    Y[m * N + n0 + j] = swiglu_oracle_silu(gate[j]) * up[j]; /* Eq. 3 */
+    Y[m * N + n0 + j] = swiglu_oracle_activation(act, gate[j]) * up[j]; /* Eq. 3 (act 0) */
   }
 }
 
@@ -88,9 +118,9 @@ static void unit(const uint16_t *A, const uint16_t *W1, const uint16_t *W2, doub
  * patterns (uint16), row-major, dense.  nthreads <= 0 means "all OpenMP threads".
  * Returns the number of threads used, or -1 on bad arguments.
  */
-int swiglu_oracle(const uint16_t *A, const uint16_t *W1, const uint16_t *W2, double *Y,
-                  int64_t M, int64_t N, int64_t K, int nthreads) {
-  if (M < 0 || N < 0 || K < 0) return -1;
+int swiglu_oracle_act(const uint16_t *A, const uint16_t *W1, const uint16_t *W2, double *Y,
+                      int64_t M, int64_t N, int64_t K, int act, int nthreads) {
+  if (M < 0 || N < 0 || K < 0 || act < 0 || act > 3) return -1;
   if (M == 0 || N == 0) return 0;
   if (!A && K > 0) return -1;
   if ((!W1 || !W2) && K > 0) return -1;
@@ -114,10 +144,15 @@ int swiglu_oracle(const uint16_t *A, const uint16_t *W1, const uint16_t *W2, dou
       const int64_t p = u / M, m = u % M;
       const int64_t n0 = p * PANEL;
       const int64_t n1 = (n0 + PANEL < N) ? n0 + PANEL : N;
-      unit(A, W1, W2, Y, N, K, m, n0, n1, gate, up);
+      unit(A, W1, W2, Y, N, K, m, n0, n1, gate, up, act);
     }
   }
   return used;
+}
+
+int swiglu_oracle(const uint16_t *A, const uint16_t *W1, const uint16_t *W2, double *Y,
+                  int64_t M, int64_t N, int64_t K, int nthreads) {
+  return swiglu_oracle_act(A, W1, W2, Y, M, N, K, 0, nthreads);
 }
 
 /*
@@ -125,10 +160,10 @@ int swiglu_oracle(const uint16_t *A, const uint16_t *W1, const uint16_t *W2, dou
  * (row indices into A) only.  Ysub is [count, N] fp64.  Rows are independent (Eq. 1-3
  * act row-wise on A), so Ysub[i,:] == Y[rows[i],:] of the full result.
  */
-int swiglu_oracle_rows(const uint16_t *A, const uint16_t *W1, const uint16_t *W2,
-                       double *Ysub, const int64_t *rows, int64_t count, int64_t M,
-                       int64_t N, int64_t K, int nthreads) {
-  if (M < 0 || N < 0 || K < 0 || count < 0) return -1;
+int swiglu_oracle_rows_act(const uint16_t *A, const uint16_t *W1, const uint16_t *W2,
+                           double *Ysub, const int64_t *rows, int64_t count, int64_t M,
+                           int64_t N, int64_t K, int act, int nthreads) {
+  if (M < 0 || N < 0 || K < 0 || count < 0 || act < 0 || act > 3) return -1;
   if (count == 0 || N == 0) return 0;
   if (!rows || !Ysub) return -1;
   if ((!A || !W1 || !W2) && K > 0) return -1;
@@ -153,10 +188,16 @@ int swiglu_oracle_rows(const uint16_t *A, const uint16_t *W1, const uint16_t *W2
       const int64_t n0 = p * PANEL;
       const int64_t n1 = (n0 + PANEL < N) ? n0 + PANEL : N;
       /* write row i of Ysub from row rows[i] of A: shift the base pointers accordingly */
-      unit(A + rows[i] * K, W1, W2, Ysub + i * N, N, K, 0, n0, n1, gate, up);
+      unit(A + rows[i] * K, W1, W2, Ysub + i * N, N, K, 0, n0, n1, gate, up, act);
     }
   }
   return used;
+}
+
+int swiglu_oracle_rows(const uint16_t *A, const uint16_t *W1, const uint16_t *W2,
+                       double *Ysub, const int64_t *rows, int64_t count, int64_t M,
+                       int64_t N, int64_t K, int nthreads) {
+  return swiglu_oracle_rows_act(A, W1, W2, Ysub, rows, count, M, N, K, 0, nthreads);
 }
 
 int swiglu_oracle_max_threads(void) {

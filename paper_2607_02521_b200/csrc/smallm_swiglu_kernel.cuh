@@ -53,15 +53,6 @@ struct SmallParams {
 #endif
 };
 
-#ifdef SWIGLU_TRACE
-#define SWIGLU_TRACE_POINT(i)                                                         \
-  do {                                                                                \
-    if (p.trace) p.trace[(size_t)blockIdx.x * 16 + (i)] = globaltimer_ns();           \
-  } while (0)
-#else
-#define SWIGLU_TRACE_POINT(i) do { } while (0)
-#endif
-
 __device__ __forceinline__ float4 ld_dsmem_v4(uint32_t cluster_addr) {
   float4 v;
   asm volatile("ld.shared::cluster.v4.f32 {%0, %1, %2, %3}, [%4];"
