@@ -95,6 +95,32 @@ int swiglu_mlp_unfused_ex(const void* A, const void* W1, const void* W2, void* Y
                           int variant, void* stream);
 
 /*
+ * Other gated activations of the GLU family ("gated linear unit variants
+ * (GEGLU, SwiGLU, ReGLU)"; line 392 future-work item 4): Y = bf16(act(A.W1) * (A.W2)) with the
+ * same tensors, layout, numeric contract (fp32 activation on the fp32 accumulators, one RNE
+ * rounding) and dispatch as swiglu_mlp.  SWIGLU_ACT_SILU makes these identical to swiglu_mlp /
+ * swiglu_mlp_unfused.  An unknown activation id returns SWIGLU_ERR_UNSUPPORTED.
+ */
+typedef enum {
+  SWIGLU_ACT_SILU = 0,      /* x * sigma(x)                       SwiGLU (the paper's Eq. 3)   */
+  SWIGLU_ACT_GELU = 1,      /* x * Phi(x) = x/2 * erfc(-x/sqrt 2) GeGLU, exact form            */
+  SWIGLU_ACT_GELU_TANH = 2, /* x/2 * (1 + tanh(sqrt(2/pi) (x + 0.044715 x^3)))  GeGLU, tanh form */
+  SWIGLU_ACT_RELU = 3       /* max(x, 0)                          ReGLU                        */
+} swiglu_activation;
+
+int swiglu_glu_mlp(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
+                   int64_t K, int activation, void* stream);
+int swiglu_glu_mlp_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                           int64_t N, int64_t K, int activation, void* stream);
+/* Forced fused variant (-1 = automatic); no fused variant needs a workspace. */
+int swiglu_glu_mlp_ex(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                      int64_t N, int64_t K, int activation, int variant, void* stream);
+/* Elementwise stage with a chosen activation: Y[i] = bf16(act(G[i]) * U[i]); see swiglu_silu_mul. */
+int swiglu_act_mul(const void* G, const void* U, void* Y, int64_t elems, int activation,
+                   void* stream);
+const char* swiglu_activation_name(int activation); /* "silu", "gelu", ...; NULL for a bad id */
+
+/*
  * The elementwise stage of the unfused path on its own (read Gate,
  * read Up, write Y; the "standalone SwiGLU" the paper profiles for its effective bandwidth,
  * line 321): Y[i] = bf16(SiLU(float(G[i])) * float(U[i])) for i < elems.  G, U, Y: device

@@ -26,6 +26,8 @@ SWIGLU_ERR_CUDA = 8
 
 EXPORTS = (
     "swiglu_mlp", "swiglu_mlp_unfused", "swiglu_mlp_ex", "swiglu_mlp_unfused_ex", "swiglu_silu_mul",
+    "swiglu_glu_mlp", "swiglu_glu_mlp_unfused", "swiglu_glu_mlp_ex", "swiglu_act_mul",
+    "swiglu_activation_name",
     "swiglu_workspace_bytes", "swiglu_num_variants", "swiglu_variant_name",
     "swiglu_selected_variant", "swiglu_launches_per_call", "swiglu_validate",
     "swiglu_mlp_host", "swiglu_last_error", "swiglu_status_string", "swiglu_version",
@@ -66,6 +68,13 @@ def load():
     lib.swiglu_validate.argtypes, lib.swiglu_validate.restype = [p, p, p, p, i64, i64, i64], ci
     lib.swiglu_mlp_host.argtypes, lib.swiglu_mlp_host.restype = [p, p, p, p, i64, i64, i64, ci, p], ci
     lib.swiglu_silu_mul.argtypes, lib.swiglu_silu_mul.restype = [p, p, p, i64, p], ci
+    lib.swiglu_act_mul.argtypes, lib.swiglu_act_mul.restype = [p, p, p, i64, ci, p], ci
+    for name in ("swiglu_glu_mlp", "swiglu_glu_mlp_unfused"):
+        f = getattr(lib, name)
+        f.argtypes, f.restype = [p, p, p, p, i64, i64, i64, ci, p], ci
+    lib.swiglu_glu_mlp_ex.argtypes = [p, p, p, p, i64, i64, i64, ci, ci, p]
+    lib.swiglu_glu_mlp_ex.restype = ci
+    lib.swiglu_activation_name.argtypes, lib.swiglu_activation_name.restype = [ci], ctypes.c_char_p
     lib.swiglu_last_error.argtypes, lib.swiglu_last_error.restype = [], ctypes.c_char_p
     lib.swiglu_status_string.argtypes, lib.swiglu_status_string.restype = [ci], ctypes.c_char_p
     lib.swiglu_version.argtypes, lib.swiglu_version.restype = [], ctypes.c_char_p
@@ -150,6 +159,45 @@ def swiglu_mlp_unfused_ex(A, W1, W2, Y, M=None, N=None, K=None, workspace=None,
     _check(load().swiglu_mlp_unfused_ex(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), m, n, k,
                                         _ptr(workspace), int(workspace_bytes), int(variant),
                                         _stream(stream)))
+
+
+ACTIVATIONS = {"silu": 0, "gelu": 1, "gelu_tanh": 2, "relu": 3}   # swiglu_activation ids
+
+
+def _act(activation) -> int:
+    return int(ACTIVATIONS.get(activation, activation))
+
+
+def swiglu_glu_mlp(A, W1, W2, Y, activation, M=None, N=None, K=None, stream=None) -> None:
+    """Y = bf16(act(A.W1) * (A.W2)), act = "silu" | "gelu" | "gelu_tanh" | "relu" (or its id)."""
+    m, n, k = _dims(A, W1, W2, Y, M, N, K)
+    _check(load().swiglu_glu_mlp(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), m, n, k, _act(activation),
+                                 _stream(stream)))
+
+
+def swiglu_glu_mlp_unfused(A, W1, W2, Y, activation, M=None, N=None, K=None, stream=None) -> None:
+    m, n, k = _dims(A, W1, W2, Y, M, N, K)
+    _check(load().swiglu_glu_mlp_unfused(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), m, n, k,
+                                         _act(activation), _stream(stream)))
+
+
+def swiglu_glu_mlp_ex(A, W1, W2, Y, activation, variant=-1, M=None, N=None, K=None,
+                      stream=None) -> None:
+    m, n, k = _dims(A, W1, W2, Y, M, N, K)
+    _check(load().swiglu_glu_mlp_ex(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), m, n, k,
+                                    _act(activation), int(variant), _stream(stream)))
+
+
+def swiglu_act_mul(G, U, Y, activation, elems=None, stream=None) -> None:
+    if elems is None:
+        elems = int(G.numel())
+    _check(load().swiglu_act_mul(_ptr(G), _ptr(U), _ptr(Y), int(elems), _act(activation),
+                                 _stream(stream)))
+
+
+def swiglu_activation_name(activation: int):
+    r = load().swiglu_activation_name(int(activation))
+    return r.decode() if r else None
 
 
 def swiglu_silu_mul(G, U, Y, elems=None, stream=None) -> None:

@@ -118,7 +118,45 @@ __device__ __forceinline__ void decode_tile_w(const GemmParams& p, int t, int& t
   }
 }
 
-template <int kCtaGroup, bool kFused, int kBN = 128>
+// Gate activations of the GLU family (include/swiglu_mlp.h swiglu_activation; PAPER.md line 56
+// and line 392 item 4).  All in fp32 on the fp32 accumulators, like SiLU (line 370).
+enum : int { kActSilu = 0, kActGelu = 1, kActGeluTanh = 2, kActRelu = 3, kNumActs = 4 };
+
+template <int kAct>
+__device__ __forceinline__ float glu_mul(float g, float u) {
+  if constexpr (kAct == kActSilu) {
+    return silu_mul(g, u);
+  } else if constexpr (kAct == kActGeluTanh) {
+    // 0.5 g (1 + tanh(c (g + 0.044715 g^3))) = g * sigma(2c (g + 0.044715 g^3)): the SiLU
+    // form with a cubic argument -- no cancellation in the negative tail.
+    const float z = g * fmaf(0.07135481627f, g * g, 1.5957691216f);  // 2c*0.044715, 2c
+    float e, r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(z * -1.4426950408889634f));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
+    return (g * u) * r;
+  } else if constexpr (kAct == kActGelu) {
+    // g * Phi(g), Phi(g) = erfc(-g / sqrt 2) / 2.  erfc(t), t >= 0, from Abramowitz & Stegun
+    // 7.1.26: (a1 k + ... + a5 k^5) exp(-t^2), k = 1 / (1 + 0.3275911 t), |error| <= 1.5e-7 --
+    // fp32-epsilon level where Phi ~ 1, and |g u| * 1.5e-7 is far below the 2e-3 absolute
+    // floor of the tolerance in the tail.  2 MUFU + ~10 FMA per element (libm erfcf is ~5x that
+    // and does not hide under the next tile's MMAs).
+    const float t = fabsf(g) * 0.70710678118654752f;
+    float k, e;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(k) : "f"(fmaf(0.3275911f, t, 1.0f)));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(t * t * -1.4426950408889634f));
+    float q = fmaf(1.061405429f, k, -1.453152027f);
+    q = fmaf(q, k, 1.421413741f);
+    q = fmaf(q, k, -0.284496736f);
+    q = fmaf(q, k, 0.254829592f);
+    q = 0.5f * (q * k) * e;                       // Phi(-|g|)
+    const float phi = (g < 0.0f) ? q : 1.0f - q;  // Phi(g)
+    return (g * u) * phi;
+  } else {
+    return fmaxf(g, 0.0f) * u;
+  }
+}
+
+template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = kActSilu>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                    const __grid_constant__ CUtensorMap tmap_b1,
@@ -325,9 +363,10 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
             tmem_ld_wait();
 #pragma unroll
             for (int j = 0; j < 16; ++j) {
-              const float y0 = silu_mul(__uint_as_float(g[2 * j]), __uint_as_float(u[2 * j]));
+              const float y0 =
+                  glu_mul<kAct>(__uint_as_float(g[2 * j]), __uint_as_float(u[2 * j]));
               const float y1 =
-                  silu_mul(__uint_as_float(g[2 * j + 1]), __uint_as_float(u[2 * j + 1]));
+                  glu_mul<kAct>(__uint_as_float(g[2 * j + 1]), __uint_as_float(u[2 * j + 1]));
               packed[j] = pack_bf16x2_rn(y0, y1);
             }
           } else {
@@ -382,6 +421,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
 // Elementwise stage of the unfused path: Y = bf16( SiLU(float(G)) * float(U) )
 // (read Gate, read Up, write Y).  16-byte vector accesses.
 // ---------------------------------------------------------------------------------------
+template <int kAct>
 __global__ void __launch_bounds__(256)
 silu_mul_kernel(const uint4* __restrict__ G, const uint4* __restrict__ U, uint4* __restrict__ Y,
                 int64_t n_vec) {
@@ -395,7 +435,7 @@ silu_mul_kernel(const uint4* __restrict__ G, const uint4* __restrict__ U, uint4*
     for (int j = 0; j < 4; ++j) {
       const float g0 = __uint_as_float(gw[j] << 16), g1 = __uint_as_float(gw[j] & 0xFFFF0000u);
       const float u0 = __uint_as_float(uw[j] << 16), u1 = __uint_as_float(uw[j] & 0xFFFF0000u);
-      yw[j] = pack_bf16x2_rn(silu_mul(g0, u0), silu_mul(g1, u1));
+      yw[j] = pack_bf16x2_rn(glu_mul<kAct>(g0, u0), glu_mul<kAct>(g1, u1));
     }
     Y[i] = make_uint4(yw[0], yw[1], yw[2], yw[3]);
   }

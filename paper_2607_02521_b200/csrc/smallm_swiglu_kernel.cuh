@@ -62,7 +62,7 @@ __device__ __forceinline__ float4 ld_dsmem_v4(uint32_t cluster_addr) {
   return v;
 }
 
-template <int MP>
+template <int MP, int kAct = kActSilu>
 __global__ void __launch_bounds__(kSmallThreads, SmallCfg<MP>::kCtasPerSm)
 smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                      const __grid_constant__ CUtensorMap tmap_w1,
@@ -253,8 +253,8 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
         }
       }
       if (n < p.N) {  // N % 8 == 0 and n % 4 == 0: the 4 columns are in range together
-        const uint32_t lo = pack_bf16x2_rn(silu_mul(gs.x, us.x), silu_mul(gs.y, us.y));
-        const uint32_t hi = pack_bf16x2_rn(silu_mul(gs.z, us.z), silu_mul(gs.w, us.w));
+        const uint32_t lo = pack_bf16x2_rn(glu_mul<kAct>(gs.x, us.x), glu_mul<kAct>(gs.y, us.y));
+        const uint32_t hi = pack_bf16x2_rn(glu_mul<kAct>(gs.z, us.z), glu_mul<kAct>(gs.w, us.w));
         *reinterpret_cast<uint2*>(Y + (long long)m * p.ldy + n) = make_uint2(lo, hi);
       }
     }

@@ -138,6 +138,21 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 EncodeTiledFn g_encode = nullptr;
 
+// Opt every fused kernel of activation kAct in to its dynamic shared-memory size.
+template <int kAct>
+int set_smem_attrs() {
+  using namespace swiglu;
+  const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+  CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true, 128, kAct>, attr, GemmCfg<1>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true, 64, kAct>, attr, GemmCfg<1, 128>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, true, 128, kAct>, attr, GemmCfg<2>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kAct>, attr, SmallCfg<16>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kAct>, attr, SmallCfg<32>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kAct>, attr, SmallCfg<64>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<128, kAct>, attr, SmallCfg<128>::kSmemBytes));
+  return SWIGLU_OK;
+}
+
 int get_device_state(DeviceState** out) {
   int dev = 0;
   CUDA_TRY(cudaGetDevice(&dev));
@@ -162,33 +177,16 @@ int get_device_state(DeviceState** out) {
       g_encode = (EncodeTiledFn)fn;
     }
     using namespace swiglu;
-    CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  GemmCfg<1>::kSmemBytes));
-    CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true, 64>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  GemmCfg<1, 128>::kSmemBytes));
+    int rc;
+    if ((rc = set_smem_attrs<kActSilu>()) || (rc = set_smem_attrs<kActGelu>()) ||
+        (rc = set_smem_attrs<kActGeluTanh>()) || (rc = set_smem_attrs<kActRelu>()))
+      return rc;
     CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, false>,
                                   cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   GemmCfg<1>::kSmemBytes));
-    CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, true>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  GemmCfg<2>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, false>,
                                   cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   GemmCfg<2>::kSmemBytes));
-    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  SmallCfg<16>::kSmemBytes));
-    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  SmallCfg<32>::kSmemBytes));
-    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  SmallCfg<64>::kSmemBytes));
-    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<128>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  SmallCfg<128>::kSmemBytes));
     d.ready = true;
   }
   *out = &d;
@@ -219,7 +217,7 @@ bool pdl_enabled() {
 }
 
 // ------------------------------------------------------------------ launches
-template <int kCtaGroup, bool kFused, int kBN = 128>
+template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = swiglu::kActSilu>
 int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void* B2, void* Yout,
                 int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
   using namespace swiglu;
@@ -285,8 +283,8 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   }
   cfg.attrs = attrs;
   cfg.numAttrs = na;
-  CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_swiglu_kernel<kCtaGroup, kFused, kBN>, ta, tb1, tb2, ty,
-                              p));
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_swiglu_kernel<kCtaGroup, kFused, kBN, kAct>, ta, tb1, tb2,
+                              ty, p));
   return SWIGLU_OK;
 }
 
@@ -315,7 +313,7 @@ int smallm_ksplit(int sm_count, int ctas_per_sm, int mp, int64_t n_tiles, int64_
   return (int)s;
 }
 
-template <int MP>
+template <int MP, int kAct>
 int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const void* W2,
                      void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
   using namespace swiglu;
@@ -360,20 +358,22 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   }
   cfg.attrs = attrs;
   cfg.numAttrs = na;
-  CUDA_TRY(cudaLaunchKernelEx(&cfg, smallm_swiglu_kernel<MP>, ta, tw1, tw2, (uint16_t*)Y, p));
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, smallm_swiglu_kernel<MP, kAct>, ta, tw1, tw2, (uint16_t*)Y, p));
   return SWIGLU_OK;
 }
 
+template <int kAct>
 int launch_smallm(const DeviceState& d, const void* A, const void* W1, const void* W2, void* Y,
                   int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
-  if (M <= 16) return launch_smallm_mp<16>(d, A, W1, W2, Y, M, N, K, stream);
-  if (M <= 32) return launch_smallm_mp<32>(d, A, W1, W2, Y, M, N, K, stream);
-  if (M <= 64) return launch_smallm_mp<64>(d, A, W1, W2, Y, M, N, K, stream);
-  return launch_smallm_mp<128>(d, A, W1, W2, Y, M, N, K, stream);
+  if (M <= 16) return launch_smallm_mp<16, kAct>(d, A, W1, W2, Y, M, N, K, stream);
+  if (M <= 32) return launch_smallm_mp<32, kAct>(d, A, W1, W2, Y, M, N, K, stream);
+  if (M <= 64) return launch_smallm_mp<64, kAct>(d, A, W1, W2, Y, M, N, K, stream);
+  return launch_smallm_mp<128, kAct>(d, A, W1, W2, Y, M, N, K, stream);
 }
 
-int launch_silu_mul(const DeviceState& d, const void* G, const void* U, void* Y, int64_t elems,
-                    cudaStream_t stream) {
+template <int kAct>
+int launch_act_mul(const DeviceState& d, const void* G, const void* U, void* Y, int64_t elems,
+                   cudaStream_t stream) {
   const int64_t n_vec = elems / 8;  // N % 8 == 0 so M*N % 8 == 0
   int64_t blocks = (n_vec + 255) / 256;
   const int64_t cap = (int64_t)d.sm_count * 8;
@@ -393,9 +393,20 @@ int launch_silu_mul(const DeviceState& d, const void* G, const void* U, void* Y,
   }
   cfg.attrs = attrs;
   cfg.numAttrs = na;
-  CUDA_TRY(cudaLaunchKernelEx(&cfg, swiglu::silu_mul_kernel, (const uint4*)G, (const uint4*)U,
-                              (uint4*)Y, n_vec));
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, swiglu::silu_mul_kernel<kAct>, (const uint4*)G,
+                              (const uint4*)U, (uint4*)Y, n_vec));
   return SWIGLU_OK;
+}
+int launch_silu_mul(const DeviceState& d, const void* G, const void* U, void* Y, int64_t elems,
+                    int act, cudaStream_t stream) {
+  using namespace swiglu;
+  switch (act) {
+    case kActSilu: return launch_act_mul<kActSilu>(d, G, U, Y, elems, stream);
+    case kActGelu: return launch_act_mul<kActGelu>(d, G, U, Y, elems, stream);
+    case kActGeluTanh: return launch_act_mul<kActGeluTanh>(d, G, U, Y, elems, stream);
+    case kActRelu: return launch_act_mul<kActRelu>(d, G, U, Y, elems, stream);
+  }
+  return fail(SWIGLU_ERR_UNSUPPORTED, "unknown activation %d", act);
 }
 
 size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -430,10 +441,24 @@ int ensure_workspace(DeviceState& d, size_t need, cudaStream_t stream, void** ou
   return SWIGLU_OK;
 }
 
+template <int kAct>
+int launch_fused(const DeviceState& d, int variant, const void* A, const void* W1, const void* W2,
+                 void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
+  switch (variant) {
+    case kFused1Cta: return launch_gemm<1, true, 128, kAct>(d, A, W1, W2, Y, M, N, K, stream);
+    case kFused2Cta: return launch_gemm<2, true, 128, kAct>(d, A, W1, W2, Y, M, N, K, stream);
+    case kFusedSmallM: return launch_smallm<kAct>(d, A, W1, W2, Y, M, N, K, stream);
+    case kFused1CtaN64: return launch_gemm<1, true, 64, kAct>(d, A, W1, W2, Y, M, N, K, stream);
+  }
+  return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
+}
+
 int run_fused(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
-              int64_t K, int variant, cudaStream_t stream) {
+              int64_t K, int variant, int act, cudaStream_t stream) {
   int rc = validate(A, W1, W2, Y, M, N, K);
   if (rc) return rc;
+  if (act < 0 || act >= swiglu::kNumActs)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "unknown activation %d", act);
   if (variant < -1 || variant >= kNumFused)
     return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
   if (variant == kFusedSmallM && M > swiglu::kSmallMMax)
@@ -443,20 +468,23 @@ int run_fused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
   DeviceState* d;
   if ((rc = get_device_state(&d))) return rc;
   if (variant < 0) variant = select_fused(M, N, K);
-  switch (variant) {
-    case kFused1Cta: return launch_gemm<1, true>(*d, A, W1, W2, Y, M, N, K, stream);
-    case kFused2Cta: return launch_gemm<2, true>(*d, A, W1, W2, Y, M, N, K, stream);
-    case kFusedSmallM: return launch_smallm(*d, A, W1, W2, Y, M, N, K, stream);
-    case kFused1CtaN64: return launch_gemm<1, true, 64>(*d, A, W1, W2, Y, M, N, K, stream);
+  using namespace swiglu;
+  switch (act) {
+    case kActSilu: return launch_fused<kActSilu>(*d, variant, A, W1, W2, Y, M, N, K, stream);
+    case kActGelu: return launch_fused<kActGelu>(*d, variant, A, W1, W2, Y, M, N, K, stream);
+    case kActGeluTanh: return launch_fused<kActGeluTanh>(*d, variant, A, W1, W2, Y, M, N, K, stream);
+    case kActRelu: return launch_fused<kActRelu>(*d, variant, A, W1, W2, Y, M, N, K, stream);
   }
-  return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
+  return fail(SWIGLU_ERR_UNSUPPORTED, "unknown activation %d", act);
 }
 
 int run_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
-                int64_t K, void* ws, size_t ws_bytes, bool own_ws, int variant,
+                int64_t K, void* ws, size_t ws_bytes, bool own_ws, int variant, int act,
                 cudaStream_t stream) {
   int rc = validate(A, W1, W2, Y, M, N, K);
   if (rc) return rc;
+  if (act < 0 || act >= swiglu::kNumActs)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "unknown activation %d", act);
   if (variant < -1 || variant >= kNumUnfused)
     return fail(SWIGLU_ERR_UNSUPPORTED, "unknown unfused variant %d", variant);
   if (M == 0) return SWIGLU_OK;
@@ -478,7 +506,7 @@ int run_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t 
     if ((rc = launch_gemm<2, false>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
     if ((rc = launch_gemm<2, false>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
   }
-  return launch_silu_mul(*d, G, U, Y, M * N, stream);
+  return launch_silu_mul(*d, G, U, Y, M * N, act, stream);
 }
 
 }  // namespace
@@ -493,29 +521,63 @@ int swiglu_validate(const void* A, const void* W1, const void* W2, const void* Y
 
 int swiglu_mlp(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
                int64_t K, void* stream) {
-  return run_fused(A, W1, W2, Y, M, N, K, -1, (cudaStream_t)stream);
+  return run_fused(A, W1, W2, Y, M, N, K, -1, swiglu::kActSilu, (cudaStream_t)stream);
 }
 
 int swiglu_mlp_ex(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
                   int64_t K, void* workspace, size_t workspace_bytes, int variant,
                   void* stream) {
   (void)workspace; (void)workspace_bytes;  // no fused variant needs a global workspace
-  return run_fused(A, W1, W2, Y, M, N, K, variant, (cudaStream_t)stream);
+  return run_fused(A, W1, W2, Y, M, N, K, variant, swiglu::kActSilu, (cudaStream_t)stream);
 }
 
 int swiglu_mlp_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
                        int64_t N, int64_t K, void* stream) {
-  return run_unfused(A, W1, W2, Y, M, N, K, nullptr, 0, true, -1, (cudaStream_t)stream);
+  return run_unfused(A, W1, W2, Y, M, N, K, nullptr, 0, true, -1, swiglu::kActSilu,
+                     (cudaStream_t)stream);
 }
 
 int swiglu_mlp_unfused_ex(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
                           int64_t N, int64_t K, void* workspace, size_t workspace_bytes,
                           int variant, void* stream) {
   return run_unfused(A, W1, W2, Y, M, N, K, workspace, workspace_bytes, false, variant,
+                     swiglu::kActSilu, (cudaStream_t)stream);
+}
+
+int swiglu_glu_mlp(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
+                   int64_t K, int activation, void* stream) {
+  return run_fused(A, W1, W2, Y, M, N, K, -1, activation, (cudaStream_t)stream);
+}
+
+int swiglu_glu_mlp_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                           int64_t N, int64_t K, int activation, void* stream) {
+  return run_unfused(A, W1, W2, Y, M, N, K, nullptr, 0, true, -1, activation,
                      (cudaStream_t)stream);
 }
 
+int swiglu_glu_mlp_ex(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                      int64_t N, int64_t K, int activation, int variant, void* stream) {
+  return run_fused(A, W1, W2, Y, M, N, K, variant, activation, (cudaStream_t)stream);
+}
+
+const char* swiglu_activation_name(int activation) {
+  switch (activation) {
+    case SWIGLU_ACT_SILU: return "silu";
+    case SWIGLU_ACT_GELU: return "gelu";
+    case SWIGLU_ACT_GELU_TANH: return "gelu_tanh";
+    case SWIGLU_ACT_RELU: return "relu";
+  }
+  return nullptr;
+}
+
 int swiglu_silu_mul(const void* G, const void* U, void* Y, int64_t elems, void* stream) {
+  return swiglu_act_mul(G, U, Y, elems, SWIGLU_ACT_SILU, stream);
+}
+
+int swiglu_act_mul(const void* G, const void* U, void* Y, int64_t elems, int activation,
+                   void* stream) {
+  if (activation < 0 || activation >= swiglu::kNumActs)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "unknown activation %d", activation);
   if (elems < 0) return fail(SWIGLU_ERR_BAD_SHAPE, "elems=%lld < 0", (long long)elems);
   if (elems % 8) return fail(SWIGLU_ERR_UNSUPPORTED, "elems=%lld must be a multiple of 8", (long long)elems);
   if (elems == 0) return SWIGLU_OK;
@@ -525,7 +587,7 @@ int swiglu_silu_mul(const void* G, const void* U, void* Y, int64_t elems, void* 
   DeviceState* d;
   int rc = get_device_state(&d);
   if (rc) return rc;
-  return launch_silu_mul(*d, G, U, Y, elems, (cudaStream_t)stream);
+  return launch_silu_mul(*d, G, U, Y, elems, activation, (cudaStream_t)stream);
 }
 
 size_t swiglu_workspace_bytes(int64_t M, int64_t N, int64_t K, int unfused, int variant) {

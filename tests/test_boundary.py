@@ -43,6 +43,17 @@ def test_version_status_strings_and_variant_table(lib):
     assert B.swiglu_launches_per_call(0, 4864, 896) == 0
 
 
+def test_activation_table(lib):
+    assert [B.swiglu_activation_name(i) for i in range(5)] == ["silu", "gelu", "gelu_tanh", "relu", None]
+    assert B.ACTIVATIONS == {"silu": 0, "gelu": 1, "gelu_tanh": 2, "relu": 3}
+    # validation precedes any CUDA call for the activation entry points too
+    rc = lib.swiglu_glu_mlp(0x10000000, 0x20000000, 0x30000000, 0x40000000, 4, 12, 8, 0, None)
+    assert rc == B.SWIGLU_ERR_UNSUPPORTED            # N % 8 != 0
+    rc = lib.swiglu_glu_mlp(0x10000000, 0x20000000, 0x30000000, 0x40000000, 4, 16, 8, 7, None)
+    assert rc == B.SWIGLU_ERR_UNSUPPORTED            # unknown activation
+    assert lib.swiglu_act_mul(0x10, 0x20, 0x30, 16, 5, None) == B.SWIGLU_ERR_UNSUPPORTED
+
+
 def test_workspace_query(lib):
     assert B.swiglu_workspace_bytes(128, 8960, 1536, unfused=False) == 0
     need = B.swiglu_workspace_bytes(128, 8960, 1536, unfused=True)

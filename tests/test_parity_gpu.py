@@ -159,6 +159,71 @@ def test_baseline_full_sizes_sampled_rows(shape):
             del dY
 
 
+ACTS = ["gelu", "gelu_tanh", "relu"]
+
+
+@pytest.mark.parametrize("act", ACTS)
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("M,N,K", [(16, 392, 328), (100, 1160, 200), (128, 4864, 896)])
+def test_other_gated_activations_every_fused_variant(act, variant, M, N, K):
+    """GeGLU (erf and tanh forms) and ReGLU through every fused kernel, std chosen so Gate
+    spans roughly [-6, 6] (both tails of the activation)."""
+    A, W1, W2 = inputs.make_case(M, N, K, seed=500 + M + N, std=0.1)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2, act=act)
+    dA, dW1, dW2 = dev(A), dev(W1), dev(W2)
+    dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+    B.swiglu_glu_mlp_ex(dA, dW1, dW2, dY, act, variant=variant)
+    torch.cuda.synchronize()
+    assert_parity(host(dY), y_ref, (act, variant, M, N, K))
+
+
+@pytest.mark.parametrize("act", ["silu"] + ACTS)
+def test_gated_activations_auto_dispatch_and_unfused(act):
+    """Automatic dispatch (small-M, 64-column, 2-CTA kernels) and the unfused path, per
+    activation; "silu" through swiglu_glu_mlp must be bit-identical to swiglu_mlp."""
+    K, N, seed, _ = inputs.SHAPES["qwen2.5-0.5b"]
+    W1, W2 = inputs.make_weights(K, N, seed)
+    A_all = inputs.make_activations(300, K, seed)
+    dW1, dW2 = dev(W1), dev(W2)
+    for M in (7, 100, 300):
+        A = A_all[:M]
+        y_ref, _ = oracle.swiglu_oracle(A, W1, W2, act=act)
+        dA = dev(A)
+        dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+        B.swiglu_glu_mlp(dA, dW1, dW2, dY, act)
+        torch.cuda.synchronize()
+        y = host(dY)
+        assert_parity(y, y_ref, (act, "fused", M))
+        if act == "silu":
+            dY2 = torch.empty_like(dY)
+            B.swiglu_mlp(dA, dW1, dW2, dY2)
+            torch.cuda.synchronize()
+            assert np.array_equal(y, host(dY2))
+        dY.fill_(float("nan"))
+        B.swiglu_glu_mlp_unfused(dA, dW1, dW2, dY, act)
+        torch.cuda.synchronize()
+        assert_parity(host(dY), y_ref, (act, "unfused", M))
+    with pytest.raises(B.SwigluError) as e:
+        B.swiglu_glu_mlp(dA, dW1, dW2, dY, 9)
+    assert e.value.status == B.SWIGLU_ERR_UNSUPPORTED
+
+
+@pytest.mark.parametrize("act", ACTS)
+def test_elementwise_stage_other_activations(act):
+    rng = np.random.Generator(np.random.Philox(key=78))
+    n = 8 * 4001
+    g = inputs.f32_to_bf16_bits((rng.standard_normal(n) * 3).astype(np.float32))
+    u = inputs.f32_to_bf16_bits(rng.standard_normal(n).astype(np.float32))
+    g[:8] = inputs.f64_to_bf16_bits_exact([0.0, 1.0, -1.0, 40.0, -40.0, 8.0, -8.0, 0.5])
+    dG, dU = dev(g), dev(u)
+    dY = torch.full((n,), float("nan"), dtype=torch.bfloat16, device="cuda")
+    B.swiglu_act_mul(dG, dU, dY, act)
+    torch.cuda.synchronize()
+    g64, u64 = inputs.bf16_bits_to_f64(g), inputs.bf16_bits_to_f64(u)
+    y_ref = np.array([oracle.activation(act, x) for x in g64]) * u64
+    assert_parity(host(dY), y_ref, ("act_mul", act))
+
+
 def test_elementwise_stage_alone():
     """swiglu_silu_mul against the oracle's own fp64 SiLU on bf16 Gate/Up values (including
     the tails |g| up to 40 where SiLU -> g and SiLU -> 0-), ragged length (multiple of 8)."""
