@@ -115,6 +115,19 @@ int swiglu_glu_mlp_unfused(const void* A, const void* W1, const void* W2, void* 
 /* Forced fused variant (-1 = automatic); no fused variant needs a workspace. */
 int swiglu_glu_mlp_ex(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
                       int64_t N, int64_t K, int activation, int variant, void* stream);
+/*
+ * Weight layout.  SWIGLU_WEIGHTS_KN is the paper's and every other entry point's: W1, W2 are
+ * K x N row-major.  SWIGLU_WEIGHTS_NK takes them as N x K row-major
+ * (K contiguous) -- the layout nn.Linear and the serving stacks the paper targets keep their
+ * projections in (lines 72-74) -- so a checkpoint's gate_proj / up_proj can be passed as they
+ * are.  Everything else (A, Y, numeric contract, dispatch, errors) is as for swiglu_glu_mlp;
+ * `unfused` != 0 runs the comparison path, `variant` = -1 is automatic.
+ */
+typedef enum { SWIGLU_WEIGHTS_KN = 0, SWIGLU_WEIGHTS_NK = 1 } swiglu_weight_layout;
+int swiglu_glu_mlp_layout(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                          int64_t N, int64_t K, int activation, int weight_layout, int unfused,
+                          int variant, void* stream);
+
 /* Elementwise stage with a chosen activation: Y[i] = bf16(act(G[i]) * U[i]); see swiglu_silu_mul. */
 int swiglu_act_mul(const void* G, const void* U, void* Y, int64_t elems, int activation,
                    void* stream);

@@ -27,7 +27,7 @@ SWIGLU_ERR_CUDA = 8
 EXPORTS = (
     "swiglu_mlp", "swiglu_mlp_unfused", "swiglu_mlp_ex", "swiglu_mlp_unfused_ex", "swiglu_silu_mul",
     "swiglu_glu_mlp", "swiglu_glu_mlp_unfused", "swiglu_glu_mlp_ex", "swiglu_act_mul",
-    "swiglu_activation_name",
+    "swiglu_activation_name", "swiglu_glu_mlp_layout",
     "swiglu_workspace_bytes", "swiglu_num_variants", "swiglu_variant_name",
     "swiglu_selected_variant", "swiglu_launches_per_call", "swiglu_validate",
     "swiglu_mlp_host", "swiglu_last_error", "swiglu_status_string", "swiglu_version",
@@ -75,6 +75,8 @@ def load():
     lib.swiglu_glu_mlp_ex.argtypes = [p, p, p, p, i64, i64, i64, ci, ci, p]
     lib.swiglu_glu_mlp_ex.restype = ci
     lib.swiglu_activation_name.argtypes, lib.swiglu_activation_name.restype = [ci], ctypes.c_char_p
+    lib.swiglu_glu_mlp_layout.argtypes = [p, p, p, p, i64, i64, i64, ci, ci, ci, ci, p]
+    lib.swiglu_glu_mlp_layout.restype = ci
     lib.swiglu_last_error.argtypes, lib.swiglu_last_error.restype = [], ctypes.c_char_p
     lib.swiglu_status_string.argtypes, lib.swiglu_status_string.restype = [ci], ctypes.c_char_p
     lib.swiglu_version.argtypes, lib.swiglu_version.restype = [], ctypes.c_char_p
@@ -186,6 +188,21 @@ def swiglu_glu_mlp_ex(A, W1, W2, Y, activation, variant=-1, M=None, N=None, K=No
     m, n, k = _dims(A, W1, W2, Y, M, N, K)
     _check(load().swiglu_glu_mlp_ex(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), m, n, k,
                                     _act(activation), int(variant), _stream(stream)))
+
+
+WEIGHTS_KN, WEIGHTS_NK = 0, 1   # swiglu_weight_layout
+
+
+def swiglu_glu_mlp_layout(A, W1, W2, Y, activation="silu", weight_layout=WEIGHTS_NK, unfused=False,
+                          variant=-1, M=None, N=None, K=None, stream=None) -> None:
+    """As swiglu_glu_mlp with W1, W2 given as [N, K] row-major (weight_layout=WEIGHTS_NK, the
+    nn.Linear layout) or [K, N] (WEIGHTS_KN)."""
+    if M is None:
+        M, K = int(A.shape[0]), int(A.shape[1])
+        N = int(Y.shape[1])
+    _check(load().swiglu_glu_mlp_layout(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), int(M), int(N), int(K),
+                                        _act(activation), int(weight_layout), int(bool(unfused)),
+                                        int(variant), _stream(stream)))
 
 
 def swiglu_act_mul(G, U, Y, activation, elems=None, stream=None) -> None:

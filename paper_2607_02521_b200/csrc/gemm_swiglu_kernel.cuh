@@ -156,7 +156,12 @@ __device__ __forceinline__ float glu_mul(float g, float u) {
   }
 }
 
-template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = kActSilu>
+// kWK = false: weights are [K,N] row-major (N contiguous; the paper's layout, PAPER.md lines
+//   94, 206) -- an MN-major UMMA "B" operand.  kWK = true: weights are [N,K] row-major (K
+//   contiguous, the nn.Linear layout serving stacks store, lines 72-74) -- a K-major operand.
+//   Either way a 64-column slab of a weight tile is one 8 KB TMA box (64 x 64 bf16, 128-byte
+//   swizzle) and the slabs W1[0:64) W1[64:128) W2[0:64) W2[64:128) sit 8 KB apart.
+template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = kActSilu, bool kWK = false>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                    const __grid_constant__ CUtensorMap tmap_b1,
@@ -200,33 +205,37 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     }
     const int k0 = kb * BK;
     const uint32_t sa = smem_a(s), sb = smem_b(s), fb = full_bar(s);
+    // one 64-column x 64-k weight slab; the tensor map's inner dimension is N ([K,N]) or K ([N,K])
+    auto load_w = [&](uint32_t dst, const CUtensorMap* tm, int n) {
+      if constexpr (kCtaGroup == 1) tma_load_2d(dst, tm, fb, kWK ? k0 : n, kWK ? n : k0, kEvictNormal);
+      else tma_load_2d_pair(dst, tm, fb, kWK ? k0 : n, kWK ? n : k0, kEvictNormal);
+    };
     if constexpr (kCtaGroup == 1) {
       tma_load_2d(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
       if constexpr (kFused) {
-        if (kBN == 64 || half) {  // W1 atom | W2 atom
-          tma_load_2d(sb, &tmap_b1, fb, n_base, k0, kEvictNormal);
-          tma_load_2d(sb + 8192, &tmap_b2, fb, n_base, k0, kEvictNormal);
-        } else {                  // W1 atoms 0,1 | W2 atoms 0,1
-          tma_load_2d(sb, &tmap_b1, fb, n_base, k0, kEvictNormal);
-          tma_load_2d(sb + 8192, &tmap_b1, fb, n_base + 64, k0, kEvictNormal);
-          tma_load_2d(sb + 16384, &tmap_b2, fb, n_base, k0, kEvictNormal);
-          tma_load_2d(sb + 24576, &tmap_b2, fb, n_base + 64, k0, kEvictNormal);
+        if (kBN == 64 || half) {  // W1 slab | W2 slab
+          load_w(sb, &tmap_b1, n_base);
+          load_w(sb + 8192, &tmap_b2, n_base);
+        } else {                  // W1 slabs 0,1 | W2 slabs 0,1
+          load_w(sb, &tmap_b1, n_base);
+          load_w(sb + 8192, &tmap_b1, n_base + 64);
+          load_w(sb + 16384, &tmap_b2, n_base);
+          load_w(sb + 24576, &tmap_b2, n_base + 64);
         }
       } else {
 #pragma unroll
-        for (int j = 0; j < 4; ++j)
-          tma_load_2d(sb + j * 8192, &tmap_b1, fb, n_base + j * 64, k0, kEvictNormal);
+        for (int j = 0; j < 4; ++j) load_w(sb + j * 8192, &tmap_b1, n_base + j * 64);
       }
     } else {
       tma_load_2d_pair(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
       if constexpr (kFused) {
         const CUtensorMap* tb = (rank == 0) ? &tmap_b1 : &tmap_b2;
-        tma_load_2d_pair(sb, tb, fb, n_base, k0, kEvictNormal);
-        if (!half) tma_load_2d_pair(sb + 8192, tb, fb, n_base + 64, k0, kEvictNormal);
+        load_w(sb, tb, n_base);
+        if (!half) load_w(sb + 8192, tb, n_base + 64);
       } else {
         const int nb = n_base + (int)rank * 128;
-        tma_load_2d_pair(sb, &tmap_b1, fb, nb, k0, kEvictNormal);
-        tma_load_2d_pair(sb + 8192, &tmap_b1, fb, nb + 64, k0, kEvictNormal);
+        load_w(sb, &tmap_b1, nb);
+        load_w(sb + 8192, &tmap_b1, nb + 64);
       }
     }
   };
@@ -295,8 +304,8 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   } else if (warp == 1 && lane == 0 && rank == 0) {
     // ================================================================ MMA issuer
     constexpr uint32_t idesc_full = idesc_bf16_f32(BM * kCtaGroup, UMMA_N, /*a_mn=*/false,
-                                                   /*b_mn=*/true);
-    constexpr uint32_t idesc_half = idesc_bf16_f32(BM * kCtaGroup, 128, false, true);
+                                                   /*b_mn=*/!kWK);
+    constexpr uint32_t idesc_half = idesc_bf16_f32(BM * kCtaGroup, 128, false, !kWK);
     int s = 0;
     uint32_t ph = 0;
     int it = 0;
@@ -318,8 +327,10 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
         for (int k = 0; k < BK / UMMA_K; ++k) {
           // A: K-major, +32 B per 16-k step inside the 128-byte swizzle row.
           const uint64_t adesc = smem_desc_sw128(sa + k * (UMMA_K * 2), 16, 1024);
-          // B: MN-major, 16 k rows = 2 KB per step; 64-column atoms 8 KB apart.
-          const uint64_t bdesc = smem_desc_sw128(sb + k * (UMMA_K * 128), 8192, 1024);
+          // B, [K,N] weights: MN-major, 16 k rows = 2 KB per step, 64-column slabs 8 KB apart.
+          // B, [N,K] weights: K-major like A (slabs of 64 n-rows are 8 KB = 8 groups of 8 rows).
+          const uint64_t bdesc = kWK ? smem_desc_sw128(sb + k * (UMMA_K * 2), 16, 1024)
+                                     : smem_desc_sw128(sb + k * (UMMA_K * 128), 8192, 1024);
           umma_bf16<kCtaGroup>(d_tmem, adesc, bdesc, idesc, (kb | k) != 0 ? 1u : 0u);
         }
         umma_commit<kCtaGroup>(empty_bar(s));  // smem stage free once these MMAs retire

@@ -62,7 +62,7 @@ __device__ __forceinline__ float4 ld_dsmem_v4(uint32_t cluster_addr) {
   return v;
 }
 
-template <int MP, int kAct = kActSilu>
+template <int MP, int kAct = kActSilu, bool kWK = false>
 __global__ void __launch_bounds__(kSmallThreads, SmallCfg<MP>::kCtasPerSm)
 smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                      const __grid_constant__ CUtensorMap tmap_w1,
@@ -96,10 +96,14 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     mbar_arrive_expect_tx(fb, Cfg::kStageBytes);
     const int k0 = kb * BK;
     // weights are read exactly once per call: do not let them push A out of L2
-    tma_load_2d(smem_w1(s), &tmap_w1, fb, n_base, k0, kEvictFirst);
-    tma_load_2d(smem_w1(s) + 8192, &tmap_w1, fb, n_base + 64, k0, kEvictFirst);
-    tma_load_2d(smem_w2(s), &tmap_w2, fb, n_base, k0, kEvictFirst);
-    tma_load_2d(smem_w2(s) + 8192, &tmap_w2, fb, n_base + 64, k0, kEvictFirst);
+    // one 64-column x 64-k slab per load; inner tensor-map dimension is N ([K,N]) or K ([N,K])
+    auto load_w = [&](uint32_t dst, const CUtensorMap* tm, int n) {
+      tma_load_2d(dst, tm, fb, kWK ? k0 : n, kWK ? n : k0, kEvictFirst);
+    };
+    load_w(smem_w1(s), &tmap_w1, n_base);
+    load_w(smem_w1(s) + 8192, &tmap_w1, n_base + 64);
+    load_w(smem_w2(s), &tmap_w2, n_base);
+    load_w(smem_w2(s) + 8192, &tmap_w2, n_base + 64);
     tma_load_2d(smem_act(s), &tmap_a, fb, k0, 0, kEvictLast);
   };
 
@@ -121,10 +125,11 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     // L2 prefetch of this CTA's weight stream (hint; legal before griddepcontrol.wait)
     const int kb = kb_begin + (int)lane;
     if ((int)lane < p.prefetch_blocks && kb < kb_end) {
-      tma_prefetch_l2_2d(&tmap_w1, n_base, kb * BK);
-      tma_prefetch_l2_2d(&tmap_w1, n_base + 64, kb * BK);
-      tma_prefetch_l2_2d(&tmap_w2, n_base, kb * BK);
-      tma_prefetch_l2_2d(&tmap_w2, n_base + 64, kb * BK);
+      const int k0 = kb * BK;
+      tma_prefetch_l2_2d(&tmap_w1, kWK ? k0 : n_base, kWK ? n_base : k0);
+      tma_prefetch_l2_2d(&tmap_w1, kWK ? k0 : n_base + 64, kWK ? n_base + 64 : k0);
+      tma_prefetch_l2_2d(&tmap_w2, kWK ? k0 : n_base, kWK ? n_base : k0);
+      tma_prefetch_l2_2d(&tmap_w2, kWK ? k0 : n_base + 64, kWK ? n_base + 64 : k0);
     }
     if (lane == 0) {
       // A may be the previous kernel's output: real loads only after the grid dependency
@@ -154,7 +159,7 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     }
   } else if (warp == 1 && lane == 0) {
     // ================================================================ MMA issuer
-    constexpr uint32_t idesc = idesc_bf16_f32(128, MP, /*a_mn=*/true, /*b_mn=*/false);
+    constexpr uint32_t idesc = idesc_bf16_f32(128, MP, /*a_mn=*/!kWK, /*b_mn=*/false);
     int s = 0;
     uint32_t ph = 0;
     for (int kb = kb_begin; kb < kb_end; ++kb) {
@@ -165,8 +170,11 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       for (int k = 0; k < BK / UMMA_K; ++k) {
         const uint32_t acc = (kb > kb_begin || k > 0) ? 1u : 0u;
         // W tiles: MN-major "A" operand, 16 k rows = 2 KB per step, 64-column atoms 8 KB apart
-        const uint64_t w1d = smem_desc_sw128(smem_w1(s) + k * (UMMA_K * 128), 8192, 1024);
-        const uint64_t w2d = smem_desc_sw128(smem_w2(s) + k * (UMMA_K * 128), 8192, 1024);
+        // ([N,K] weights: K-major, +32 B per step, the two 64-row slabs are contiguous)
+        const uint64_t w1d = kWK ? smem_desc_sw128(smem_w1(s) + k * (UMMA_K * 2), 16, 1024)
+                                 : smem_desc_sw128(smem_w1(s) + k * (UMMA_K * 128), 8192, 1024);
+        const uint64_t w2d = kWK ? smem_desc_sw128(smem_w2(s) + k * (UMMA_K * 2), 16, 1024)
+                                 : smem_desc_sw128(smem_w2(s) + k * (UMMA_K * 128), 8192, 1024);
         // activations: K-major "B" operand, +32 B per step inside the swizzle row
         const uint64_t ad = smem_desc_sw128(smem_act(s) + k * (UMMA_K * 2), 16, 1024);
         umma_bf16<1>(tmem_base, w1d, ad, idesc, acc);       // Gate^T -> columns [0, MP)

@@ -139,17 +139,21 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 EncodeTiledFn g_encode = nullptr;
 
 // Opt every fused kernel of activation kAct in to its dynamic shared-memory size.
-template <int kAct>
+template <int kAct, bool kWK>
 int set_smem_attrs() {
   using namespace swiglu;
   const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
-  CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true, 128, kAct>, attr, GemmCfg<1>::kSmemBytes));
-  CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true, 64, kAct>, attr, GemmCfg<1, 128>::kSmemBytes));
-  CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, true, 128, kAct>, attr, GemmCfg<2>::kSmemBytes));
-  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kAct>, attr, SmallCfg<16>::kSmemBytes));
-  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kAct>, attr, SmallCfg<32>::kSmemBytes));
-  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kAct>, attr, SmallCfg<64>::kSmemBytes));
-  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<128, kAct>, attr, SmallCfg<128>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true, 128, kAct, kWK>, attr, GemmCfg<1>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true, 64, kAct, kWK>, attr, GemmCfg<1, 128>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, true, 128, kAct, kWK>, attr, GemmCfg<2>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kAct, kWK>, attr, SmallCfg<16>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kAct, kWK>, attr, SmallCfg<32>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kAct, kWK>, attr, SmallCfg<64>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<128, kAct, kWK>, attr, SmallCfg<128>::kSmemBytes));
+  if (kAct == kActSilu) {  // the unfused path's plain GEMM has no activation
+    CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, false, 128, kActSilu, kWK>, attr, GemmCfg<1>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, false, 128, kActSilu, kWK>, attr, GemmCfg<2>::kSmemBytes));
+  }
   return SWIGLU_OK;
 }
 
@@ -178,15 +182,11 @@ int get_device_state(DeviceState** out) {
     }
     using namespace swiglu;
     int rc;
-    if ((rc = set_smem_attrs<kActSilu>()) || (rc = set_smem_attrs<kActGelu>()) ||
-        (rc = set_smem_attrs<kActGeluTanh>()) || (rc = set_smem_attrs<kActRelu>()))
+    if ((rc = set_smem_attrs<kActSilu, false>()) || (rc = set_smem_attrs<kActGelu, false>()) ||
+        (rc = set_smem_attrs<kActGeluTanh, false>()) || (rc = set_smem_attrs<kActRelu, false>()) ||
+        (rc = set_smem_attrs<kActSilu, true>()) || (rc = set_smem_attrs<kActGelu, true>()) ||
+        (rc = set_smem_attrs<kActGeluTanh, true>()) || (rc = set_smem_attrs<kActRelu, true>()))
       return rc;
-    CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, false>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  GemmCfg<1>::kSmemBytes));
-    CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, false>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  GemmCfg<2>::kSmemBytes));
     d.ready = true;
   }
   *out = &d;
@@ -217,15 +217,16 @@ bool pdl_enabled() {
 }
 
 // ------------------------------------------------------------------ launches
-template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = swiglu::kActSilu>
+template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = swiglu::kActSilu, bool kWK = false>
 int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void* B2, void* Yout,
                 int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
   using namespace swiglu;
   CUtensorMap ta, tb1, tb2, ty;
   int rc;
   if ((rc = make_tmap(&ta, A, K, M, 64, 128))) return rc;
-  if ((rc = make_tmap(&tb1, B1, N, K, 64, 64))) return rc;
-  if ((rc = make_tmap(&tb2, kFused ? B2 : B1, N, K, 64, 64))) return rc;
+  // weights: [K,N] (inner N) or [N,K] (inner K); a box is always one 64 x 64 slab
+  if ((rc = make_tmap(&tb1, B1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
+  if ((rc = make_tmap(&tb2, kFused ? B2 : B1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
   if ((rc = make_tmap(&ty, Yout, N, M, 64, 128))) return rc;
   using Cfg = GemmCfg<kCtaGroup, kFused ? 2 * kBN : 256>;
   GemmParams p;
@@ -283,8 +284,8 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   }
   cfg.attrs = attrs;
   cfg.numAttrs = na;
-  CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_swiglu_kernel<kCtaGroup, kFused, kBN, kAct>, ta, tb1, tb2,
-                              ty, p));
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_swiglu_kernel<kCtaGroup, kFused, kBN, kAct, kWK>, ta, tb1,
+                              tb2, ty, p));
   return SWIGLU_OK;
 }
 
@@ -313,15 +314,15 @@ int smallm_ksplit(int sm_count, int ctas_per_sm, int mp, int64_t n_tiles, int64_
   return (int)s;
 }
 
-template <int MP, int kAct>
+template <int MP, int kAct, bool kWK>
 int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const void* W2,
                      void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
   using namespace swiglu;
   CUtensorMap ta, tw1, tw2;
   int rc;
   if ((rc = make_tmap(&ta, A, K, M, 64, MP))) return rc;
-  if ((rc = make_tmap(&tw1, W1, N, K, 64, 64))) return rc;
-  if ((rc = make_tmap(&tw2, W2, N, K, 64, 64))) return rc;
+  if ((rc = make_tmap(&tw1, W1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
+  if ((rc = make_tmap(&tw2, W2, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
   const int64_t n_tiles = (N + 127) / 128, k_blocks = (K + BK - 1) / BK;
   SmallParams p;
   p.M = (int)M; p.N = (int)N; p.K = (int)K;
@@ -358,17 +359,18 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   }
   cfg.attrs = attrs;
   cfg.numAttrs = na;
-  CUDA_TRY(cudaLaunchKernelEx(&cfg, smallm_swiglu_kernel<MP, kAct>, ta, tw1, tw2, (uint16_t*)Y, p));
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, smallm_swiglu_kernel<MP, kAct, kWK>, ta, tw1, tw2, (uint16_t*)Y,
+                              p));
   return SWIGLU_OK;
 }
 
-template <int kAct>
+template <int kAct, bool kWK>
 int launch_smallm(const DeviceState& d, const void* A, const void* W1, const void* W2, void* Y,
                   int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
-  if (M <= 16) return launch_smallm_mp<16, kAct>(d, A, W1, W2, Y, M, N, K, stream);
-  if (M <= 32) return launch_smallm_mp<32, kAct>(d, A, W1, W2, Y, M, N, K, stream);
-  if (M <= 64) return launch_smallm_mp<64, kAct>(d, A, W1, W2, Y, M, N, K, stream);
-  return launch_smallm_mp<128, kAct>(d, A, W1, W2, Y, M, N, K, stream);
+  if (M <= 16) return launch_smallm_mp<16, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
+  if (M <= 32) return launch_smallm_mp<32, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
+  if (M <= 64) return launch_smallm_mp<64, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
+  return launch_smallm_mp<128, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
 }
 
 template <int kAct>
@@ -441,20 +443,28 @@ int ensure_workspace(DeviceState& d, size_t need, cudaStream_t stream, void** ou
   return SWIGLU_OK;
 }
 
-template <int kAct>
-int launch_fused(const DeviceState& d, int variant, const void* A, const void* W1, const void* W2,
-                 void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
+template <int kAct, bool kWK>
+int launch_fused_l(const DeviceState& d, int variant, const void* A, const void* W1,
+                   const void* W2, void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
   switch (variant) {
-    case kFused1Cta: return launch_gemm<1, true, 128, kAct>(d, A, W1, W2, Y, M, N, K, stream);
-    case kFused2Cta: return launch_gemm<2, true, 128, kAct>(d, A, W1, W2, Y, M, N, K, stream);
-    case kFusedSmallM: return launch_smallm<kAct>(d, A, W1, W2, Y, M, N, K, stream);
-    case kFused1CtaN64: return launch_gemm<1, true, 64, kAct>(d, A, W1, W2, Y, M, N, K, stream);
+    case kFused1Cta: return launch_gemm<1, true, 128, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
+    case kFused2Cta: return launch_gemm<2, true, 128, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
+    case kFusedSmallM: return launch_smallm<kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
+    case kFused1CtaN64: return launch_gemm<1, true, 64, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
   }
   return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
 }
+template <int kAct>
+int launch_fused(const DeviceState& d, int variant, int layout, const void* A, const void* W1,
+                 const void* W2, void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
+  return layout ? launch_fused_l<kAct, true>(d, variant, A, W1, W2, Y, M, N, K, stream)
+                : launch_fused_l<kAct, false>(d, variant, A, W1, W2, Y, M, N, K, stream);
+}
 
 int run_fused(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
-              int64_t K, int variant, int act, cudaStream_t stream) {
+              int64_t K, int variant, int act, int layout, cudaStream_t stream) {
+  if (layout != SWIGLU_WEIGHTS_KN && layout != SWIGLU_WEIGHTS_NK)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "unknown weight layout %d", layout);
   int rc = validate(A, W1, W2, Y, M, N, K);
   if (rc) return rc;
   if (act < 0 || act >= swiglu::kNumActs)
@@ -470,17 +480,19 @@ int run_fused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
   if (variant < 0) variant = select_fused(M, N, K);
   using namespace swiglu;
   switch (act) {
-    case kActSilu: return launch_fused<kActSilu>(*d, variant, A, W1, W2, Y, M, N, K, stream);
-    case kActGelu: return launch_fused<kActGelu>(*d, variant, A, W1, W2, Y, M, N, K, stream);
-    case kActGeluTanh: return launch_fused<kActGeluTanh>(*d, variant, A, W1, W2, Y, M, N, K, stream);
-    case kActRelu: return launch_fused<kActRelu>(*d, variant, A, W1, W2, Y, M, N, K, stream);
+    case kActSilu: return launch_fused<kActSilu>(*d, variant, layout, A, W1, W2, Y, M, N, K, stream);
+    case kActGelu: return launch_fused<kActGelu>(*d, variant, layout, A, W1, W2, Y, M, N, K, stream);
+    case kActGeluTanh: return launch_fused<kActGeluTanh>(*d, variant, layout, A, W1, W2, Y, M, N, K, stream);
+    case kActRelu: return launch_fused<kActRelu>(*d, variant, layout, A, W1, W2, Y, M, N, K, stream);
   }
   return fail(SWIGLU_ERR_UNSUPPORTED, "unknown activation %d", act);
 }
 
 int run_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
                 int64_t K, void* ws, size_t ws_bytes, bool own_ws, int variant, int act,
-                cudaStream_t stream) {
+                int layout, cudaStream_t stream) {
+  if (layout != SWIGLU_WEIGHTS_KN && layout != SWIGLU_WEIGHTS_NK)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "unknown weight layout %d", layout);
   int rc = validate(A, W1, W2, Y, M, N, K);
   if (rc) return rc;
   if (act < 0 || act >= swiglu::kNumActs)
@@ -499,12 +511,19 @@ int run_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t 
   if (variant < 0) variant = select_unfused(M, N, K);
   void* G = ws;
   void* U = (char*)ws + need / 2;
-  if (variant == kUnfused1Cta) {
+  using swiglu::kActSilu;
+  if (variant == kUnfused1Cta && !layout) {
     if ((rc = launch_gemm<1, false>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
     if ((rc = launch_gemm<1, false>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
-  } else {
+  } else if (variant == kUnfused1Cta) {
+    if ((rc = launch_gemm<1, false, 128, kActSilu, true>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
+    if ((rc = launch_gemm<1, false, 128, kActSilu, true>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
+  } else if (!layout) {
     if ((rc = launch_gemm<2, false>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
     if ((rc = launch_gemm<2, false>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
+  } else {
+    if ((rc = launch_gemm<2, false, 128, kActSilu, true>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
+    if ((rc = launch_gemm<2, false, 128, kActSilu, true>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
   }
   return launch_silu_mul(*d, G, U, Y, M * N, act, stream);
 }
@@ -521,19 +540,19 @@ int swiglu_validate(const void* A, const void* W1, const void* W2, const void* Y
 
 int swiglu_mlp(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
                int64_t K, void* stream) {
-  return run_fused(A, W1, W2, Y, M, N, K, -1, swiglu::kActSilu, (cudaStream_t)stream);
+  return run_fused(A, W1, W2, Y, M, N, K, -1, swiglu::kActSilu, 0, (cudaStream_t)stream);
 }
 
 int swiglu_mlp_ex(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
                   int64_t K, void* workspace, size_t workspace_bytes, int variant,
                   void* stream) {
   (void)workspace; (void)workspace_bytes;  // no fused variant needs a global workspace
-  return run_fused(A, W1, W2, Y, M, N, K, variant, swiglu::kActSilu, (cudaStream_t)stream);
+  return run_fused(A, W1, W2, Y, M, N, K, variant, swiglu::kActSilu, 0, (cudaStream_t)stream);
 }
 
 int swiglu_mlp_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
                        int64_t N, int64_t K, void* stream) {
-  return run_unfused(A, W1, W2, Y, M, N, K, nullptr, 0, true, -1, swiglu::kActSilu,
+  return run_unfused(A, W1, W2, Y, M, N, K, nullptr, 0, true, -1, swiglu::kActSilu, 0,
                      (cudaStream_t)stream);
 }
 
@@ -541,23 +560,33 @@ int swiglu_mlp_unfused_ex(const void* A, const void* W1, const void* W2, void* Y
                           int64_t N, int64_t K, void* workspace, size_t workspace_bytes,
                           int variant, void* stream) {
   return run_unfused(A, W1, W2, Y, M, N, K, workspace, workspace_bytes, false, variant,
-                     swiglu::kActSilu, (cudaStream_t)stream);
+                     swiglu::kActSilu, 0, (cudaStream_t)stream);
 }
 
 int swiglu_glu_mlp(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
                    int64_t K, int activation, void* stream) {
-  return run_fused(A, W1, W2, Y, M, N, K, -1, activation, (cudaStream_t)stream);
+  return run_fused(A, W1, W2, Y, M, N, K, -1, activation, 0, (cudaStream_t)stream);
 }
 
 int swiglu_glu_mlp_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
                            int64_t N, int64_t K, int activation, void* stream) {
-  return run_unfused(A, W1, W2, Y, M, N, K, nullptr, 0, true, -1, activation,
+  return run_unfused(A, W1, W2, Y, M, N, K, nullptr, 0, true, -1, activation, 0,
                      (cudaStream_t)stream);
+}
+
+int swiglu_glu_mlp_layout(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                          int64_t N, int64_t K, int activation, int weight_layout, int unfused,
+                          int variant, void* stream) {
+  if (unfused)
+    return run_unfused(A, W1, W2, Y, M, N, K, nullptr, 0, true, variant, activation,
+                       weight_layout, (cudaStream_t)stream);
+  return run_fused(A, W1, W2, Y, M, N, K, variant, activation, weight_layout,
+                   (cudaStream_t)stream);
 }
 
 int swiglu_glu_mlp_ex(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
                       int64_t N, int64_t K, int activation, int variant, void* stream) {
-  return run_fused(A, W1, W2, Y, M, N, K, variant, activation, (cudaStream_t)stream);
+  return run_fused(A, W1, W2, Y, M, N, K, variant, activation, 0, (cudaStream_t)stream);
 }
 
 const char* swiglu_activation_name(int activation) {

@@ -224,6 +224,53 @@ def test_elementwise_stage_other_activations(act):
     assert_parity(host(dY), y_ref, ("act_mul", act))
 
 
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("M,N,K", [(1, 128, 64), (16, 392, 328), (100, 1160, 200), (128, 4864, 896),
+                                   (7, 136, 72)])
+def test_nk_weight_layout_every_fused_variant(variant, M, N, K):
+    """Weights handed over as [N, K] row-major (K-major UMMA operand).  The oracle sees the
+    same weights in the paper's [K, N] layout; the transposition is input preparation here."""
+    A, W1, W2 = inputs.make_case(M, N, K, seed=600 + M + N, std=0.05)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+    dA, dW1t, dW2t = dev(A), dev(np.ascontiguousarray(W1.T)), dev(np.ascontiguousarray(W2.T))
+    dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+    B.swiglu_glu_mlp_layout(dA, dW1t, dW2t, dY, "silu", B.WEIGHTS_NK, variant=variant)
+    torch.cuda.synchronize()
+    assert_parity(host(dY), y_ref, ("nk", variant, M, N, K))
+
+
+@pytest.mark.parametrize("act", ["silu", "gelu", "relu"])
+def test_nk_weight_layout_auto_unfused_and_tail_tiles(act):
+    """[N,K] weights: automatic dispatch over decode / mid / large M (incl. a shape whose last
+    wave runs as half tiles), the unfused path, and bit-identity with the [K,N] entry point."""
+    K, N = 200, 1032
+    A_all, W1, W2 = inputs.make_case(2560, N, K, seed=640, std=0.07)
+    dW1, dW2 = dev(W1), dev(W2)
+    dW1t, dW2t = dev(np.ascontiguousarray(W1.T)), dev(np.ascontiguousarray(W2.T))
+    for M in (5, 60, 128, 300, 2560):
+        A = A_all[:M]
+        y_ref, _ = oracle.swiglu_oracle(A, W1, W2, act=act)
+        dA = dev(A)
+        dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+        B.swiglu_glu_mlp_layout(dA, dW1t, dW2t, dY, act, B.WEIGHTS_NK)
+        torch.cuda.synchronize()
+        y_nk = host(dY)
+        assert_parity(y_nk, y_ref, ("nk-auto", act, M))
+        dY2 = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+        B.swiglu_glu_mlp_layout(dA, dW1, dW2, dY2, act, B.WEIGHTS_KN)
+        B.swiglu_glu_mlp(dA, dW1, dW2, dY, act)
+        torch.cuda.synchronize()
+        assert np.array_equal(host(dY2), host(dY))           # KN through the layout entry point
+        assert_parity(host(dY2), y_ref, ("kn-auto", act, M))
+        dY.fill_(float("nan"))
+        B.swiglu_glu_mlp_layout(dA, dW1t, dW2t, dY, act, B.WEIGHTS_NK, unfused=True)
+        torch.cuda.synchronize()
+        assert_parity(host(dY), y_ref, ("nk-unfused", act, M))
+    with pytest.raises(B.SwigluError) as e:
+        B.swiglu_glu_mlp_layout(dA, dW1t, dW2t, dY, act, 5)
+    assert e.value.status == B.SWIGLU_ERR_UNSUPPORTED
+
+
 def test_elementwise_stage_alone():
     """swiglu_silu_mul against the oracle's own fp64 SiLU on bf16 Gate/Up values (including
     the tails |g| up to 40 where SiLU -> g and SiLU -> 0-), ragged length (multiple of 8)."""
