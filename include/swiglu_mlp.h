@@ -27,7 +27,7 @@
  *
  * Ownership: the caller owns A, W1, W2, Y and any workspace and keeps them valid until the
  * enqueued work has completed.  The 8-argument forms may use a library-owned, lazily grown,
- * per-device workspace; growing it allocates (never while the stream is capturing -- use
+ * per-stream workspace; growing it allocates (never while the stream is capturing -- use
  * the _ex forms with a caller workspace under CUDA-graph capture).
  *
  * Errors: a swiglu_status return code; the library never throws, aborts, prints or

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <mutex>
 #include <vector>
 
@@ -124,10 +125,11 @@ struct DeviceState {
   int device = -1;
   int sm_count = 0;
   int cc_major = 0;
-  void* workspace = nullptr;
-  size_t workspace_bytes = 0;
-  void* host_scratch = nullptr;  // device scratch of swiglu_mlp_host
-  size_t host_scratch_bytes = 0;
+  // Library-owned buffers are PER STREAM: two calls on different streams may run at the same
+  // time and must not share Gate/Up workspace or staging memory.
+  struct Buf { void* ptr = nullptr; size_t bytes = 0; };
+  std::map<cudaStream_t, Buf> workspace;     // unfused path: bf16 Gate | Up
+  std::map<cudaStream_t, Buf> host_scratch;  // swiglu_mlp_host: device copies of A, W1, W2, Y
 };
 std::mutex g_mu;
 DeviceState g_dev[64];
@@ -421,25 +423,29 @@ size_t workspace_for(int64_t M, int64_t N, int64_t K, int unfused, int variant) 
   return 0;  // fused variants reduce split-K partials on chip (DSMEM), no global workspace
 }
 
-int ensure_workspace(DeviceState& d, size_t need, cudaStream_t stream, void** out) {
+// Grow-only buffer of `stream` in `pool`.  Growing waits for that stream's earlier work (which
+// may still be using the old buffer) and allocates; never while the stream is capturing.
+int ensure_stream_buffer(std::map<cudaStream_t, DeviceState::Buf>& pool, size_t need,
+                         cudaStream_t stream, void** out) {
   std::lock_guard<std::mutex> lk(g_mu);
-  if (need > d.workspace_bytes) {
+  DeviceState::Buf& b = pool[stream];
+  if (need > b.bytes) {
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     cudaStreamIsCapturing(stream, &cap);
     if (cap != cudaStreamCaptureStatusNone)
       return fail(SWIGLU_ERR_WORKSPACE,
                   "library workspace must grow to %zu bytes but the stream is capturing; "
                   "use the _ex form with a caller workspace", need);
-    if (d.workspace) {
-      CUDA_TRY(cudaDeviceSynchronize());  // earlier calls may still be using the old buffer
-      CUDA_TRY(cudaFree(d.workspace));
-      d.workspace = nullptr;
-      d.workspace_bytes = 0;
+    if (b.ptr) {
+      CUDA_TRY(cudaStreamSynchronize(stream));
+      CUDA_TRY(cudaFree(b.ptr));
+      b.ptr = nullptr;
+      b.bytes = 0;
     }
-    CUDA_TRY(cudaMalloc(&d.workspace, need));
-    d.workspace_bytes = need;
+    CUDA_TRY(cudaMalloc(&b.ptr, need));
+    b.bytes = need;
   }
-  *out = d.workspace;
+  *out = b.ptr;
   return SWIGLU_OK;
 }
 
@@ -507,7 +513,7 @@ int run_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t 
   }
   DeviceState* d;
   if ((rc = get_device_state(&d))) return rc;
-  if (own_ws && (rc = ensure_workspace(*d, need, stream, &ws))) return rc;
+  if (own_ws && (rc = ensure_stream_buffer(d->workspace, need, stream, &ws))) return rc;
   if (variant < 0) variant = select_unfused(M, N, K);
   void* G = ws;
   void* U = (char*)ws + need / 2;
@@ -655,21 +661,9 @@ int swiglu_mlp_host(const void* A_host, const void* W1_host, const void* W2_host
   const size_t ab = round_up((size_t)M * K * 2, 256), wb = round_up((size_t)K * N * 2, 256),
                yb = round_up((size_t)M * N * 2, 256);
   const size_t need = ab + 2 * wb + yb;
-  char* base;
-  {
-    std::lock_guard<std::mutex> lk(g_mu);
-    if (need > d->host_scratch_bytes) {
-      if (d->host_scratch) {
-        CUDA_TRY(cudaDeviceSynchronize());
-        CUDA_TRY(cudaFree(d->host_scratch));
-        d->host_scratch = nullptr;
-        d->host_scratch_bytes = 0;
-      }
-      CUDA_TRY(cudaMalloc(&d->host_scratch, need));
-      d->host_scratch_bytes = need;
-    }
-    base = (char*)d->host_scratch;
-  }
+  void* scratch;
+  if ((rc = ensure_stream_buffer(d->host_scratch, need, stream, &scratch))) return rc;
+  char* base = (char*)scratch;
   void *dA = base, *dW1 = base + ab, *dW2 = base + ab + wb, *dY = base + ab + 2 * wb;
   CUDA_TRY(cudaMemcpyAsync(dA, A_host, (size_t)M * K * 2, cudaMemcpyHostToDevice, stream));
   CUDA_TRY(cudaMemcpyAsync(dW1, W1_host, (size_t)K * N * 2, cudaMemcpyHostToDevice, stream));

@@ -271,6 +271,38 @@ def test_nk_weight_layout_auto_unfused_and_tail_tiles(act):
     assert e.value.status == B.SWIGLU_ERR_UNSUPPORTED
 
 
+def test_many_rows_and_concurrent_host_threads():
+    """M beyond 65535 rows (tile coordinates past 16 bits) and four host threads calling the
+    library at once on their own streams (header: entry points are thread-safe)."""
+    import threading
+    A, W1, W2 = inputs.make_case(70001, 136, 72, seed=700, std=0.1)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+    dA, dW1, dW2 = dev(A), dev(W1), dev(W2)
+    outs, errs = {}, []
+
+    def worker(i, M):
+        try:
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                dY = torch.full((M, 136), float("nan"), dtype=torch.bfloat16, device="cuda")
+                for _ in range(5):
+                    if i % 2:
+                        B.swiglu_mlp_unfused(dA[:M], dW1, dW2, dY)
+                    else:
+                        B.swiglu_mlp(dA[:M], dW1, dW2, dY)
+                st.synchronize()
+                outs[i] = (M, host(dY))
+        except Exception as e:  # noqa: BLE001
+            errs.append((i, e))
+
+    ts = [threading.Thread(target=worker, args=(i, M)) for i, M in enumerate((70001, 40000, 9, 300))]
+    [t.start() for t in ts]
+    [t.join() for t in ts]
+    assert not errs, errs
+    for i, (M, y) in outs.items():
+        assert_parity(y, y_ref[:M], ("threads", i, M))
+
+
 def test_elementwise_stage_alone():
     """swiglu_silu_mul against the oracle's own fp64 SiLU on bf16 Gate/Up values (including
     the tails |g| up to 40 where SiLU -> g and SiLU -> 0-), ragged length (multiple of 8)."""
