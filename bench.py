@@ -212,15 +212,29 @@ class Workload:
             from paper_2607_02521_b200 import binding
             raise binding.SwigluError(rc, binding.last_error())
 
+    def unfused_fn(self, M):
+        """swiglu_mlp_unfused_ex with a caller-owned Gate/Up workspace: the timing loop replays
+        a captured CUDA graph, and the library's own per-stream workspace cannot be grown
+        while a stream is capturing (include/swiglu_mlp.h)."""
+        import torch
+        from paper_2607_02521_b200 import binding as B
+        lib = B.load()
+        need = int(lib.swiglu_workspace_bytes(M, self.N, self.K, 1, -1))
+        if getattr(self, "_ws", None) is None or self._ws.numel() < need:
+            self._ws = torch.empty(max(need, 256), dtype=torch.uint8, device="cuda")
+        ws = self._ws.data_ptr()
+
+        def fn(a, w1, w2, y, m, n, k, stream):
+            return lib.swiglu_mlp_unfused_ex(a, w1, w2, y, m, n, k, ws, need, -1, stream)
+        return fn
+
     def flops_per_step(self):
         return sum(flops(M, self.N, self.K) for M in self.Ms)
 
 
-def time_point(wl, fn, M, target_ms=1.5, batches=15):
-    """Median / min microseconds per call.  A batch of back-to-back calls (rotating weight
-    copies) is captured once into a CUDA graph and replayed between two CUDA events, so the
-    figure is what a serving loop replaying a captured decode step sees, free of Python
-    launch gaps; calls >= ~100 us are not launch-bound and give the same number either way."""
+def _capture(wl, fn, M, target_ms):
+    """Warm `fn`, estimate its time, capture a whole number of weight-copy rotations of
+    back-to-back calls into a CUDA graph.  Returns (graph, calls per replay, ms per replay)."""
     import torch
     for _ in range(3):
         wl.call(fn, M)
@@ -239,20 +253,44 @@ def time_point(wl, fn, M, target_ms=1.5, batches=15):
     with torch.cuda.graph(g):
         for _ in range(per):
             wl.call(fn, M)
-    for _ in range(max(2, int(10.0 / max(est_ms * per, 1e-3)))):   # ~10 ms of warm replays
-        g.replay()
-    torch.cuda.synchronize()
-    samples = []
-    for _ in range(batches):
-        e0.record()
-        g.replay()
-        e1.record()
-        torch.cuda.synchronize()
-        samples.append(e0.elapsed_time(e1) * 1e3 / per)
+    return g, per, est_ms * per
+
+
+def _stats(samples, per, batches):
     med = statistics.median(samples)
     cv = (statistics.pstdev(samples) / med) if med > 0 else 0.0
     return {"us_median": med, "us_min": min(samples), "cv": cv, "calls_per_batch": per,
             "batches": batches}
+
+
+def time_points(wl, fns, M, target_ms=1.5, batches=15):
+    """Median / min microseconds per call for each callable in `fns`, sampled INTERLEAVED
+    (A, B, A, B, ...), so that clock / power / thermal drift during the measurement hits every
+    candidate alike and ratios between them (speed-up over unfused) are not an artefact of
+    order.  Each candidate is a batch of back-to-back calls (rotating weight copies) captured
+    once into a CUDA graph and replayed between two CUDA events: what a serving loop replaying
+    a captured decode step sees, free of Python launch gaps."""
+    import torch
+    caps = [_capture(wl, fn, M, target_ms) for fn in fns]
+    for g, per, ms in caps:
+        for _ in range(max(2, int(10.0 / max(ms, 1e-3)))):   # ~10 ms of warm replays each
+            g.replay()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    samples = [[] for _ in fns]
+    for _ in range(batches):
+        for i, (g, per, _) in enumerate(caps):
+            e0.record()
+            g.replay()
+            e1.record()
+            torch.cuda.synchronize()
+            samples[i].append(e0.elapsed_time(e1) * 1e3 / per)
+    return [_stats(s, caps[i][1], batches) for i, s in enumerate(samples)]
+
+
+def time_point(wl, fn, M, target_ms=1.5, batches=15):
+    """One callable (see time_points)."""
+    return time_points(wl, [fn], M, target_ms, batches)[0]
 
 
 def check_point(wl, M, max_rows=16):
@@ -287,8 +325,7 @@ def measure_points(wl, peaks, do_check=True, Ms=None):
     from paper_2607_02521_b200 import binding as B
     pts = []
     for M in (Ms or wl.Ms):
-        f = time_point(wl, B.load().swiglu_mlp, M)
-        u = time_point(wl, B.load().swiglu_mlp_unfused, M)
+        f, u = time_points(wl, [B.load().swiglu_mlp, wl.unfused_fn(M)], M)
         t = f["us_median"] * 1e-6
         fl, by = flops(M, wl.N, wl.K), algo_bytes(M, wl.N, wl.K)
         t_roof, bound = roofline_time_s(M, wl.N, wl.K, peaks["bf16_tflops"], peaks["hbm_gbs"])
