@@ -125,3 +125,36 @@ def test_product_path_does_not_import_the_oracle():
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2607_02521_b200" not in text
             assert "from paper_2607_02521_b200" not in text
+
+
+def test_header_is_plain_c_and_the_library_links_from_c(tmp_path):
+    """include/swiglu_mlp.h compiles as C11 (no C++ or torch types) and a C program linked
+    against the shared library can call the host-only entry points."""
+    import subprocess
+    src = tmp_path / "abi.c"
+    src.write_text(r"""
+#include <stdio.h>
+#include "swiglu_mlp.h"
+int main(void) {
+  printf("%s\n", swiglu_version());
+  printf("%d %d\n", swiglu_num_variants(0), swiglu_num_variants(1));
+  printf("%s\n", swiglu_variant_name(0, swiglu_selected_variant(16, 4864, 896, 0)));
+  printf("%d\n", swiglu_validate((void*)16, (void*)32, (void*)48, (void*)64, 4, 12, 8));
+  printf("%d\n", swiglu_mlp(0, 0, 0, 0, 0, 16, 8, 0));          /* M == 0: OK, no launch */
+  printf("%s\n", swiglu_activation_name(SWIGLU_ACT_GELU_TANH));
+  printf("%zu\n", swiglu_workspace_bytes(128, 8960, 1536, 1, -1));
+  return 0;
+}
+""")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    pkg = os.path.join(root, "paper_2607_02521_b200")
+    exe = tmp_path / "abi"
+    subprocess.run(["gcc", "-std=c11", "-Wall", "-Wextra", "-Werror", "-pedantic",
+                    "-I", os.path.join(root, "include"), str(src), "-o", str(exe),
+                    "-L", pkg, "-l:libswiglu_b200.so", f"-Wl,-rpath,{pkg}"], check=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split("\n")
+    assert "sm_100a" in out[0]
+    assert out[1].split() == [str(B.swiglu_num_variants(False)), str(B.swiglu_num_variants(True))]
+    assert "smallm" in out[2]
+    assert int(out[3]) == B.SWIGLU_ERR_UNSUPPORTED and int(out[4]) == B.SWIGLU_OK
+    assert out[5] == "gelu_tanh" and int(out[6]) >= 2 * 128 * 8960 * 2
