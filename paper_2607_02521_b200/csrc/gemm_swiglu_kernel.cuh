@@ -56,6 +56,7 @@ struct GemmParams {
   int wide_tiles;   // tiles [0, wide_tiles) are full width; the rest are 64-column half tiles
   int total_tiles;  // wide_tiles + 2 * (m_tiles*n_tiles - wide_tiles)
   int early_issue;      // 1: fill the ring before the CTA-wide setup barrier (small grids)
+  int w_evict_first;    // 1: weights are read once (one row of tiles): L2 evict-first loads
 #ifdef SWIGLU_TRACE
   unsigned long long* trace;  // [grid][kGemmTraceStride] globaltimer stamps (debug builds only)
 #endif
@@ -195,6 +196,8 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   const int total_tiles = p.total_tiles;
   const int k_blocks = (p.K + BK - 1) / BK;
 
+  // A single row of tiles reads every weight byte exactly once: stream it past L2 (evict-first).
+  const uint64_t w_policy = p.w_evict_first ? kEvictFirst : kEvictNormal;
   // One k-block of A and B into ring slot s (no waiting here: the caller owns the ring state).
   // w = output columns of the tile (kOutCols, or 64 for a half tile of the last wave).
   auto issue_loads = [&](int s, int kb, int m_base, int n_base, int w) {
@@ -207,8 +210,8 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     const uint32_t sa = smem_a(s), sb = smem_b(s), fb = full_bar(s);
     // one 64-column x 64-k weight slab; the tensor map's inner dimension is N ([K,N]) or K ([N,K])
     auto load_w = [&](uint32_t dst, const CUtensorMap* tm, int n) {
-      if constexpr (kCtaGroup == 1) tma_load_2d(dst, tm, fb, kWK ? k0 : n, kWK ? n : k0, kEvictNormal);
-      else tma_load_2d_pair(dst, tm, fb, kWK ? k0 : n, kWK ? n : k0, kEvictNormal);
+      if constexpr (kCtaGroup == 1) tma_load_2d(dst, tm, fb, kWK ? k0 : n, kWK ? n : k0, w_policy);
+      else tma_load_2d_pair(dst, tm, fb, kWK ? k0 : n, kWK ? n : k0, w_policy);
     };
     if constexpr (kCtaGroup == 1) {
       tma_load_2d(sa, &tmap_a, fb, k0, m_base, kEvictNormal);

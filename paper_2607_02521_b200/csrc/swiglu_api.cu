@@ -260,6 +260,7 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   }
   // one tile per CTA (a short, HBM-bound call): fill the TMA ring before the setup barrier
   p.early_issue = (kCtaGroup == 1 && kFused && tiles <= groups && !env_int("SWIGLU_NO_EARLY", 0));
+  p.w_evict_first = (p.m_tiles == 1 && !env_int("SWIGLU_NO_W_EVICT_FIRST", 0));
 #ifdef SWIGLU_TRACE
   p.trace = g_trace;
 #endif
