@@ -271,6 +271,45 @@ def test_nk_weight_layout_auto_unfused_and_tail_tiles(act):
     assert e.value.status == B.SWIGLU_ERR_UNSUPPORTED
 
 
+@pytest.mark.parametrize("M,N,K", [(1, 8, 8), (7, 136, 72), (129, 264, 200), (300, 1032, 136),
+                                   (2305, 1160, 64)])
+def test_no_write_outside_y_or_workspace(M, N, K):
+    """Own bounds check (compute-sanitizer is closed on this GPU pool): Y and the unfused
+    workspace sit between guard bands of a sentinel pattern; every kernel variant (tail tiles,
+    clipped TMA stores, ragged M/N/K) must leave the guards untouched and write all of Y."""
+    A, W1, W2 = inputs.make_case(M, N, K, seed=800 + M, std=0.05)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+    dA, dW1, dW2 = dev(A), dev(W1), dev(W2)
+    guard = 4096                                         # elements on each side
+    SENT = -21846                                        # 0xAAAA as int16: a bf16 nobody computes
+
+    def banded(n_elems):
+        buf = torch.full((guard + n_elems + guard,), SENT, dtype=torch.int16, device="cuda")
+        return buf, buf[guard:guard + n_elems]
+
+    def guards_intact(buf, n_elems):
+        return bool((buf[:guard] == SENT).all()) and bool((buf[guard + n_elems:] == SENT).all())
+
+    for variant in range(B.swiglu_num_variants(False)):
+        if "smallm" in B.swiglu_variant_name(variant) and M > 128:
+            continue
+        ybuf, yv = banded(M * N)
+        dY = yv.view(torch.bfloat16).view(M, N)
+        B.swiglu_mlp_ex(dA, dW1, dW2, dY, variant=variant)
+        torch.cuda.synchronize()
+        assert guards_intact(ybuf, M * N), ("fused", variant)
+        assert_parity(host(dY), y_ref, ("guarded", variant, M, N, K))
+    need = B.swiglu_workspace_bytes(M, N, K, unfused=True)
+    for variant in range(B.swiglu_num_variants(True)):
+        ybuf, yv = banded(M * N)
+        wbuf, wv = banded(need // 2)
+        dY = yv.view(torch.bfloat16).view(M, N)
+        B.swiglu_mlp_unfused_ex(dA, dW1, dW2, dY, workspace=wv, workspace_bytes=need, variant=variant)
+        torch.cuda.synchronize()
+        assert guards_intact(ybuf, M * N) and guards_intact(wbuf, need // 2), ("unfused", variant)
+        assert_parity(host(dY), y_ref, ("guarded-unfused", variant, M, N, K))
+
+
 def test_many_rows_and_concurrent_host_threads():
     """M beyond 65535 rows (tile coordinates past 16 bits) and four host threads calling the
     library at once on their own streams (header: entry points are thread-safe)."""
