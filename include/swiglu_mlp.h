@@ -167,6 +167,20 @@ int swiglu_validate(const void* A, const void* W1, const void* W2, const void* Y
 int swiglu_mlp_host(const void* A_host, const void* W1_host, const void* W2_host,
                     void* Y_host, int64_t M, int64_t N, int64_t K, int unfused, void* stream);
 
+/*
+ * Host-buffer batch form: ONE pair of weight matrices and `count` activation batches that share
+ * them (the batches of one serving step).  A_host[i] is M[i] x K bf16, Y_host[i] is M[i] x N
+ * bf16; all HOST pointers (pinned memory gives copy/compute overlap; pageable works).  The
+ * weights cross PCIe once per call, in column chunks: while the kernels of chunk j run on
+ * `stream`, chunk j+1 is uploaded and chunk j-1's output columns are downloaded on internal
+ * copy streams (output columns are independent, Eq. 1-3).  Synchronises before
+ * returning; not capturable.  Device scratch is library-owned (per stream); concurrent calls
+ * on one device are serialised.  M[i] == 0 batches are skipped.
+ */
+int swiglu_mlp_host_batched(const void* const* A_host, void* const* Y_host, const int64_t* M,
+                            int count, const void* W1_host, const void* W2_host, int64_t N,
+                            int64_t K, int unfused, void* stream);
+
 /* Message for the calling thread's most recent non-OK return; static/thread-local storage. */
 const char* swiglu_last_error(void);
 const char* swiglu_status_string(int status);

@@ -27,7 +27,7 @@ SWIGLU_ERR_CUDA = 8
 EXPORTS = (
     "swiglu_mlp", "swiglu_mlp_unfused", "swiglu_mlp_ex", "swiglu_mlp_unfused_ex", "swiglu_silu_mul",
     "swiglu_glu_mlp", "swiglu_glu_mlp_unfused", "swiglu_glu_mlp_ex", "swiglu_act_mul",
-    "swiglu_activation_name", "swiglu_glu_mlp_layout",
+    "swiglu_activation_name", "swiglu_glu_mlp_layout", "swiglu_mlp_host_batched",
     "swiglu_workspace_bytes", "swiglu_num_variants", "swiglu_variant_name",
     "swiglu_selected_variant", "swiglu_launches_per_call", "swiglu_validate",
     "swiglu_mlp_host", "swiglu_last_error", "swiglu_status_string", "swiglu_version",
@@ -77,6 +77,8 @@ def load():
     lib.swiglu_activation_name.argtypes, lib.swiglu_activation_name.restype = [ci], ctypes.c_char_p
     lib.swiglu_glu_mlp_layout.argtypes = [p, p, p, p, i64, i64, i64, ci, ci, ci, ci, p]
     lib.swiglu_glu_mlp_layout.restype = ci
+    lib.swiglu_mlp_host_batched.argtypes = [p, p, p, ci, p, p, i64, i64, ci, p]
+    lib.swiglu_mlp_host_batched.restype = ci
     lib.swiglu_last_error.argtypes, lib.swiglu_last_error.restype = [], ctypes.c_char_p
     lib.swiglu_status_string.argtypes, lib.swiglu_status_string.restype = [ci], ctypes.c_char_p
     lib.swiglu_version.argtypes, lib.swiglu_version.restype = [], ctypes.c_char_p
@@ -228,6 +230,18 @@ def swiglu_mlp_host(A_host, W1_host, W2_host, Y_host, M, N, K, unfused=False, st
     """Host-buffer form: H2D copies, the kernel(s), D2H copy and a stream sync, all inside."""
     _check(load().swiglu_mlp_host(_ptr(A_host), _ptr(W1_host), _ptr(W2_host), _ptr(Y_host),
                                   int(M), int(N), int(K), int(bool(unfused)), _stream(stream)))
+
+
+def swiglu_mlp_host_batched(A_hosts, Y_hosts, Ms, W1_host, W2_host, N, K, unfused=False,
+                            stream=None) -> None:
+    """One set of host weights, several host activation batches: weights cross PCIe once, in
+    column chunks pipelined with the kernels and the downloads (see the header)."""
+    n = len(Ms)
+    a = (ctypes.c_void_p * n)(*[_ptr(x) for x in A_hosts])
+    y = (ctypes.c_void_p * n)(*[_ptr(x) for x in Y_hosts])
+    m = (ctypes.c_int64 * n)(*[int(v) for v in Ms])
+    _check(load().swiglu_mlp_host_batched(a, y, m, n, _ptr(W1_host), _ptr(W2_host), int(N), int(K),
+                                          int(bool(unfused)), _stream(stream)))
 
 
 def swiglu_validate(A, W1, W2, Y, M, N, K) -> int:

@@ -130,6 +130,10 @@ struct DeviceState {
   struct Buf { void* ptr = nullptr; size_t bytes = 0; };
   std::map<cudaStream_t, Buf> workspace;     // unfused path: bf16 Gate | Up
   std::map<cudaStream_t, Buf> host_scratch;  // swiglu_mlp_host: device copies of A, W1, W2, Y
+  // swiglu_mlp_host_batched: copy streams and events of its H2D / compute / D2H pipeline
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  cudaEvent_t ev_a = nullptr, ev_in[2] = {nullptr, nullptr}, ev_cmp[2] = {nullptr, nullptr},
+              ev_out[2] = {nullptr, nullptr};
 };
 std::mutex g_mu;
 DeviceState g_dev[64];
@@ -673,6 +677,118 @@ int swiglu_mlp_host(const void* A_host, const void* W1_host, const void* W2_host
                : swiglu_mlp(dA, dW1, dW2, dY, M, N, K, stream_v);
   if (rc) return rc;
   CUDA_TRY(cudaMemcpyAsync(Y_host, dY, (size_t)M * N * 2, cudaMemcpyDeviceToHost, stream));
+  CUDA_TRY(cudaStreamSynchronize(stream));
+  return SWIGLU_OK;
+}
+
+int swiglu_mlp_host_batched(const void* const* A_host, void* const* Y_host, const int64_t* M,
+                            int count, const void* W1_host, const void* W2_host, int64_t N,
+                            int64_t K, int unfused, void* stream_v) {
+  cudaStream_t stream = (cudaStream_t)stream_v;
+  if (count < 0) return fail(SWIGLU_ERR_BAD_SHAPE, "count=%d < 0", count);
+  if (N <= 0 || K <= 0 || (K % 8) || (N % 8))
+    return validate(nullptr, nullptr, nullptr, nullptr, 0, N, K);
+  if (count == 0) return SWIGLU_OK;
+  if (!A_host || !Y_host || !M || !W1_host || !W2_host)
+    return fail(SWIGLU_ERR_NULL_POINTER, "a host pointer is NULL");
+  int64_t rows = 0;
+  for (int i = 0; i < count; ++i) {
+    if (M[i] < 0 || M[i] > INT32_MAX - 256)
+      return fail(SWIGLU_ERR_BAD_SHAPE, "bad batch size M[%d]=%lld", i, (long long)M[i]);
+    if (M[i] > 0 && (!A_host[i] || !Y_host[i]))
+      return fail(SWIGLU_ERR_NULL_POINTER, "A_host[%d] or Y_host[%d] is NULL", i, i);
+    rows += M[i];
+  }
+  if (rows == 0) return SWIGLU_OK;
+  DeviceState* d;
+  int rc = get_device_state(&d);
+  if (rc) return rc;
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(stream, &cap);
+  if (cap != cudaStreamCaptureStatusNone)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "the host-buffer forms synchronise; not capturable");
+  // One pipeline per device at a time (it owns the copy streams and events below).
+  static std::mutex host_mu;
+  std::lock_guard<std::mutex> host_lk(host_mu);
+  if (!d->s_in) {
+    CUDA_TRY(cudaStreamCreateWithFlags(&d->s_in, cudaStreamNonBlocking));
+    CUDA_TRY(cudaStreamCreateWithFlags(&d->s_out, cudaStreamNonBlocking));
+    CUDA_TRY(cudaEventCreateWithFlags(&d->ev_a, cudaEventDisableTiming));
+    for (int b = 0; b < 2; ++b) {
+      CUDA_TRY(cudaEventCreateWithFlags(&d->ev_in[b], cudaEventDisableTiming));
+      CUDA_TRY(cudaEventCreateWithFlags(&d->ev_cmp[b], cudaEventDisableTiming));
+      CUDA_TRY(cudaEventCreateWithFlags(&d->ev_out[b], cudaEventDisableTiming));
+    }
+  }
+  // Column chunks of the weights: H2D of chunk j+1 and D2H of chunk j-1 run under the kernels
+  // of chunk j (the path has no dependency between output columns).
+  const int want_chunks = env_int("SWIGLU_HOST_CHUNKS", 4) > 0 ? env_int("SWIGLU_HOST_CHUNKS", 4) : 4;
+  int64_t nc = round_up((size_t)((N + want_chunks - 1) / want_chunks), 128);
+  if (nc < 512) nc = 512;
+  if (nc > N) nc = N;
+  const int chunks = (int)((N + nc - 1) / nc);
+  const size_t a_bytes = round_up((size_t)rows * K * 2, 256);
+  const size_t w_bytes = round_up((size_t)K * nc * 2, 256);
+  const size_t y_bytes = round_up((size_t)rows * nc * 2, 256);
+  void* scratch;
+  if ((rc = ensure_stream_buffer(d->host_scratch, a_bytes + 4 * w_bytes + 2 * y_bytes, stream,
+                                 &scratch)))
+    return rc;
+  char* dA = (char*)scratch;
+  char* dW = dA + a_bytes;                // [2 buffers][W1c | W2c]
+  char* dY = dW + 4 * w_bytes;            // [2 buffers][rows x nc]
+  // everything the caller enqueued on `stream` so far comes first
+  CUDA_TRY(cudaEventRecord(d->ev_a, stream));
+  CUDA_TRY(cudaStreamWaitEvent(d->s_in, d->ev_a, 0));
+  CUDA_TRY(cudaStreamWaitEvent(d->s_out, d->ev_a, 0));
+  {
+    size_t off = 0;
+    for (int i = 0; i < count; ++i) {
+      if (M[i] == 0) continue;
+      CUDA_TRY(cudaMemcpyAsync(dA + off, A_host[i], (size_t)M[i] * K * 2, cudaMemcpyHostToDevice,
+                               d->s_in));
+      off += (size_t)M[i] * K * 2;
+    }
+  }
+  for (int j = 0; j < chunks; ++j) {
+    const int b = j & 1;
+    const int64_t n0 = (int64_t)j * nc, ncj = (n0 + nc <= N) ? nc : N - n0;
+    char* w1c = dW + (size_t)b * 2 * w_bytes;
+    char* w2c = w1c + w_bytes;
+    char* yc = dY + (size_t)b * y_bytes;
+    // H2D: the weight columns [n0, n0 + ncj), packed dense [K, ncj]
+    if (j >= 2) CUDA_TRY(cudaStreamWaitEvent(d->s_in, d->ev_cmp[b], 0));  // buffer b consumed
+    CUDA_TRY(cudaMemcpy2DAsync(w1c, (size_t)ncj * 2, (const char*)W1_host + n0 * 2, (size_t)N * 2,
+                               (size_t)ncj * 2, (size_t)K, cudaMemcpyHostToDevice, d->s_in));
+    CUDA_TRY(cudaMemcpy2DAsync(w2c, (size_t)ncj * 2, (const char*)W2_host + n0 * 2, (size_t)N * 2,
+                               (size_t)ncj * 2, (size_t)K, cudaMemcpyHostToDevice, d->s_in));
+    CUDA_TRY(cudaEventRecord(d->ev_in[b], d->s_in));
+    // compute on the caller's stream
+    CUDA_TRY(cudaStreamWaitEvent(stream, d->ev_in[b], 0));
+    if (j >= 2) CUDA_TRY(cudaStreamWaitEvent(stream, d->ev_out[b], 0));  // Y buffer b drained
+    size_t a_off = 0, y_off = 0;
+    for (int i = 0; i < count; ++i) {
+      if (M[i] == 0) continue;
+      rc = unfused ? swiglu_mlp_unfused(dA + a_off, w1c, w2c, yc + y_off, M[i], ncj, K, stream_v)
+                   : swiglu_mlp(dA + a_off, w1c, w2c, yc + y_off, M[i], ncj, K, stream_v);
+      if (rc) return rc;
+      a_off += (size_t)M[i] * K * 2;
+      y_off += round_up((size_t)M[i] * ncj * 2, 256);
+    }
+    CUDA_TRY(cudaEventRecord(d->ev_cmp[b], stream));
+    // D2H: scatter the chunk's columns into each batch's Y
+    CUDA_TRY(cudaStreamWaitEvent(d->s_out, d->ev_cmp[b], 0));
+    y_off = 0;
+    for (int i = 0; i < count; ++i) {
+      if (M[i] == 0) continue;
+      CUDA_TRY(cudaMemcpy2DAsync((char*)Y_host[i] + n0 * 2, (size_t)N * 2, yc + y_off,
+                                 (size_t)ncj * 2, (size_t)ncj * 2, (size_t)M[i],
+                                 cudaMemcpyDeviceToHost, d->s_out));
+      y_off += round_up((size_t)M[i] * ncj * 2, 256);
+    }
+    CUDA_TRY(cudaEventRecord(d->ev_out[b], d->s_out));
+  }
+  CUDA_TRY(cudaStreamSynchronize(d->s_out));
   CUDA_TRY(cudaStreamSynchronize(stream));
   return SWIGLU_OK;
 }

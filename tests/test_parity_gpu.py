@@ -410,6 +410,30 @@ def test_host_buffer_entry_point():
         assert_parity(Y, y_ref, ("host", unfused))
 
 
+@pytest.mark.parametrize("unfused", [False, True])
+def test_host_batched_entry_point(unfused):
+    """Several host batches sharing one pair of host weights (column-chunk pipeline: N spans
+    four chunks with a ragged last one; an empty batch is skipped); pinned and pageable."""
+    K, N = 200, 4360
+    Ms = [5, 0, 130, 1, 300]
+    A_all, W1, W2 = inputs.make_case(sum(Ms), N, K, seed=900, std=0.05)
+    y_ref, _ = oracle.swiglu_oracle(A_all, W1, W2)
+    offs = np.cumsum([0] + Ms)
+    for pinned in (True, False):
+        mk = (lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int16)).pin_memory()) if pinned \
+            else (lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int16).copy()))
+        hA = [mk(A_all[offs[i]:offs[i + 1]]) if Ms[i] else None for i in range(len(Ms))]
+        hY = [mk(np.full((Ms[i], N), 0x7FC0, dtype=np.uint16)) if Ms[i] else None for i in range(len(Ms))]
+        hW1, hW2 = mk(W1), mk(W2)
+        st = torch.cuda.Stream()
+        B.swiglu_mlp_host_batched(hA, hY, Ms, hW1, hW2, N, K, unfused=unfused, stream=st)
+        for i, M in enumerate(Ms):
+            if M:
+                y = hY[i].numpy().view(np.uint16)
+                assert_parity(y, y_ref[offs[i]:offs[i + 1]], ("host_batched", unfused, pinned, i))
+    B.swiglu_mlp_host_batched([], [], [], hW1, hW2, N, K)          # count == 0: OK, nothing to do
+
+
 def test_non_default_stream_and_cuda_graph_replay():
     M, N, K = 16, 4864, 896
     A, W1, W2 = inputs.make_case(M, N, K, seed=61)
