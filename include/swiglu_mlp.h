@@ -26,12 +26,17 @@
  * Every compute entry point is asynchronous: it returns after enqueueing on `stream`.
  *
  * Ownership: the caller owns A, W1, W2, Y and any workspace and keeps them valid until the
- * enqueued work has completed.  The 8-argument forms may use a library-owned, lazily grown,
- * per-stream workspace; growing it allocates (never while the stream is capturing -- use
- * the _ex forms with a caller workspace under CUDA-graph capture).
+ * enqueued work has completed.  swiglu_mlp_unfused (8-argument form) and the host-buffer forms
+ * use a library-owned, lazily grown, PER-STREAM device buffer.  It is allocated and regrown
+ * with stream-ordered allocation (cudaMallocAsync / cudaFreeAsync on `stream`), so growth never
+ * synchronises and never frees memory that earlier work on that stream still uses.  A stream
+ * that is being captured is refused (SWIGLU_ERR_WORKSPACE): use the _ex forms with a caller
+ * workspace under CUDA-graph capture.  swiglu_release_stream / swiglu_release give the buffers
+ * back.  The fused entry points need no workspace and are always capturable.
  *
- * Errors: a swiglu_status return code; the library never throws, aborts, prints or
- * synchronises.  Argument validation happens before any CUDA call, so the validation
+ * Errors: a swiglu_status return code; the library never throws, aborts or prints, and the
+ * device-pointer compute entry points never synchronise (the host-buffer forms and
+ * swiglu_release do, and say so).  Argument validation happens before any CUDA call, so the validation
  * codes (1-5) can be exercised on a host without a GPU.  M == 0 is SWIGLU_OK and launches
  * nothing.  There is NO CPU fallback: without an sm_100 device the compute entry points
  * return SWIGLU_ERR_ARCH or SWIGLU_ERR_CUDA.
@@ -73,7 +78,9 @@ int swiglu_mlp(const void* A, const void* W1, const void* W2, void* Y, int64_t M
 /*
  * Unfused comparison path (two GEMMs that write Gate and Up
  * to HBM as bf16, then an elementwise SiLU-multiply kernel).  Built from this library's own
- * tcgen05 GEMM and elementwise kernels, no cuBLAS.  Needs 2*M*N*2 bytes of workspace
+ * tcgen05 GEMM and elementwise kernels, no cuBLAS.  For M <= 128 the two GEMMs are one merged
+ * Gate|Up launch of the same swap-AB split-K streaming kernel the fused path uses (so the
+ * comparison isolates fusion, not tile shapes).  Needs 2*M*N*2 bytes of workspace
  * (library-owned in this form).
  */
 int swiglu_mlp_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
@@ -146,7 +153,9 @@ int swiglu_silu_mul(const void* G, const void* U, void* Y, int64_t elems, void* 
  * `unfused` != 0 asks about swiglu_mlp_unfused. */
 size_t swiglu_workspace_bytes(int64_t M, int64_t N, int64_t K, int unfused, int variant);
 
-/* Variant table (fused: unfused == 0).  Names are static strings; NULL for a bad id. */
+/* Variant table (fused: unfused == 0).  Names are static strings; NULL for a bad id.
+ * (SURVEY.md 8(b) proposed these three without the `unfused` argument; the unfused path has
+ * its own variant table, so the argument selects which table is meant.) */
 int swiglu_num_variants(int unfused);
 const char* swiglu_variant_name(int unfused, int variant);
 /* The variant `-1` resolves to for this shape (host-only table lookup, no CUDA call). */
@@ -180,6 +189,43 @@ int swiglu_mlp_host(const void* A_host, const void* W1_host, const void* W2_host
 int swiglu_mlp_host_batched(const void* const* A_host, void* const* Y_host, const int64_t* M,
                             int count, const void* W1_host, const void* W2_host, int64_t N,
                             int64_t K, int unfused, void* stream);
+
+/*
+ * Library-owned memory ("workspace ... mutex-guarded").
+ * swiglu_release_stream: stream-ordered free of the buffers the library keeps for `stream` on
+ *   the current device (call it before destroying a stream you passed to swiglu_mlp_unfused or
+ *   a host-buffer form; a later stream that reuses the handle simply allocates afresh).  Does
+ *   not synchronise.
+ * swiglu_release: cudaDeviceSynchronize(), then frees every library-owned buffer, copy stream
+ *   and event of the current device.  The library stays usable; the next call re-allocates.
+ */
+int swiglu_release_stream(void* stream);
+int swiglu_release(void);
+
+/*
+ * Experiment overrides (SWIGLU_VARIANT, SWIGLU_UNFUSED_VARIANT, SWIGLU_KSPLIT, SWIGLU_GROUP_M,
+ * SWIGLU_HOST_CHUNKS, SWIGLU_NO_PDL, SWIGLU_NO_PREFETCH, SWIGLU_NO_EARLY, SWIGLU_NO_TAIL_SPLIT,
+ * SWIGLU_NO_W_EVICT_FIRST, SWIGLU_NO_TMAP_CACHE) are read from the environment once, at the
+ * first call into the library.  swiglu_reload_env re-reads them (sweeps and tests; not
+ * thread-safe against concurrent compute calls).
+ */
+void swiglu_reload_env(void);
+
+/*
+ * Measurement aid ("log the SM clock during each run"): while a device buffer
+ * of two uint64 is registered here, CTA 0 of every GEMM-class kernel this library launches
+ * (fused, unfused GEMMs; not the elementwise kernel) overwrites it at exit with
+ * {SM cycles elapsed, nanoseconds elapsed (%globaltimer)} between its entry and exit, so
+ * cycles / ns is the SM clock in GHz that launch really ran at.  Process-wide; NULL switches it
+ * off.  The caller owns the buffer and keeps it valid while launches (or captured graphs) that
+ * saw it may run.
+ */
+void swiglu_set_clock_probe(void* device_u64x2);
+
+/* Calling thread's tensor-map cache counters (a0: CUtensorMaps are encoded once per distinct
+ * (pointer, shape, box) and fetched from a thread-local cache afterwards); returns the number
+ * of cache slots.  Either pointer may be NULL. */
+int swiglu_tensor_map_cache_stats(uint64_t* hits, uint64_t* misses);
 
 /* Message for the calling thread's most recent non-OK return; static/thread-local storage. */
 const char* swiglu_last_error(void);

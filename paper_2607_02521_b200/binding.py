@@ -31,6 +31,8 @@ EXPORTS = (
     "swiglu_workspace_bytes", "swiglu_num_variants", "swiglu_variant_name",
     "swiglu_selected_variant", "swiglu_launches_per_call", "swiglu_validate",
     "swiglu_mlp_host", "swiglu_last_error", "swiglu_status_string", "swiglu_version",
+    "swiglu_release", "swiglu_release_stream", "swiglu_reload_env", "swiglu_tensor_map_cache_stats",
+    "swiglu_set_clock_probe",
 )
 
 
@@ -79,6 +81,12 @@ def load():
     lib.swiglu_glu_mlp_layout.restype = ci
     lib.swiglu_mlp_host_batched.argtypes = [p, p, p, ci, p, p, i64, i64, ci, p]
     lib.swiglu_mlp_host_batched.restype = ci
+    lib.swiglu_release.argtypes, lib.swiglu_release.restype = [], ci
+    lib.swiglu_release_stream.argtypes, lib.swiglu_release_stream.restype = [p], ci
+    lib.swiglu_reload_env.argtypes, lib.swiglu_reload_env.restype = [], None
+    u64p = ctypes.POINTER(ctypes.c_uint64)
+    lib.swiglu_tensor_map_cache_stats.argtypes, lib.swiglu_tensor_map_cache_stats.restype = [u64p, u64p], ci
+    lib.swiglu_set_clock_probe.argtypes, lib.swiglu_set_clock_probe.restype = [p], None
     lib.swiglu_last_error.argtypes, lib.swiglu_last_error.restype = [], ctypes.c_char_p
     lib.swiglu_status_string.argtypes, lib.swiglu_status_string.restype = [ci], ctypes.c_char_p
     lib.swiglu_version.argtypes, lib.swiglu_version.restype = [], ctypes.c_char_p
@@ -268,6 +276,34 @@ def swiglu_selected_variant(M, N, K, unfused=False) -> int:
 
 def swiglu_launches_per_call(M, N, K, unfused=False, variant=-1) -> int:
     return int(load().swiglu_launches_per_call(int(M), int(N), int(K), int(bool(unfused)), int(variant)))
+
+
+def swiglu_release() -> None:
+    """Synchronise the device and free every library-owned buffer, copy stream and event."""
+    _check(load().swiglu_release())
+
+
+def swiglu_release_stream(stream=None) -> None:
+    """Stream-ordered free of the library's buffers for `stream` (no synchronisation)."""
+    _check(load().swiglu_release_stream(_stream(stream)))
+
+
+def swiglu_reload_env() -> None:
+    """Re-read the SWIGLU_* experiment overrides from the environment (sweeps / tests)."""
+    load().swiglu_reload_env()
+
+
+def swiglu_tensor_map_cache_stats():
+    """(hits, misses, slots) of the calling thread's tensor-map cache."""
+    h, m = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    slots = load().swiglu_tensor_map_cache_stats(ctypes.byref(h), ctypes.byref(m))
+    return int(h.value), int(m.value), int(slots)
+
+
+def swiglu_set_clock_probe(buf) -> None:
+    """Register (or, with None, clear) a device buffer of two uint64 {SM cycles, ns} that CTA 0
+    of every GEMM-class launch fills in; see the header."""
+    load().swiglu_set_clock_probe(_ptr(buf))
 
 
 def last_error() -> str:

@@ -57,6 +57,7 @@ struct GemmParams {
   int total_tiles;  // wide_tiles + 2 * (m_tiles*n_tiles - wide_tiles)
   int early_issue;      // 1: fill the ring before the CTA-wide setup barrier (small grids)
   int w_evict_first;    // 1: weights are read once (one row of tiles): L2 evict-first loads
+  unsigned long long* clk;  // optional {SM cycles, globaltimer ns} of CTA 0 (swiglu_set_clock_probe)
 #ifdef SWIGLU_TRACE
   unsigned long long* trace;  // [grid][kGemmTraceStride] globaltimer stamps (debug builds only)
 #endif
@@ -246,6 +247,10 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
 
   // ------------------------------------------------------------------ one-time setup
   if (threadIdx.x == 0) SWIGLU_GEMM_TRACE(0);
+  const bool clk_probe = p.clk != nullptr && blockIdx.x == 0 && threadIdx.x == 0;
+  long long clk_c0 = 0;
+  uint64_t clk_t0 = 0;
+  if (clk_probe) { clk_c0 = clock64(); clk_t0 = globaltimer_ns(); }
   if (warp == 0) {
     if (lane == 0) {
       prefetch_tensormap(&tmap_a);
@@ -429,6 +434,10 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     tmem_dealloc<kCtaGroup>(tmem_base, kTmemCols);
   }
   if (threadIdx.x == 0) SWIGLU_GEMM_TRACE(2);
+  if (clk_probe) {
+    p.clk[0] = (unsigned long long)(clock64() - clk_c0);
+    p.clk[1] = globaltimer_ns() - clk_t0;
+  }
 }
 
 // ---------------------------------------------------------------------------------------

@@ -48,6 +48,8 @@ struct SmallParams {
   int ksplit;         // cluster size S
   int prefetch_blocks;  // leading k-blocks of each CTA's weight stream to prefetch into L2
   long long ldy;      // = N
+  uint16_t* U;        // kStoreGU only: bf16 Up output (Gate goes to the Y argument)
+  unsigned long long* clk;  // optional {SM cycles, globaltimer ns} of CTA 0 (swiglu_set_clock_probe)
 #ifdef SWIGLU_TRACE
   unsigned long long* trace;  // [grid][16] globaltimer stamps (debug builds only)
 #endif
@@ -62,7 +64,11 @@ __device__ __forceinline__ float4 ld_dsmem_v4(uint32_t cluster_addr) {
   return v;
 }
 
-template <int MP, int kAct = kActSilu, bool kWK = false>
+// kStoreGU = true: the merged Gate|Up GEMM of the UNFUSED comparison path at decode sizes (a7):
+//   the reduced fp32 Gate and Up are each rounded to bf16 and written to HBM (Y argument = Gate,
+//   p.U = Up) instead of going through the activation -- one launch for both projections, the
+//   "merged gate_up_proj" serving stacks run before their silu_and_mul kernel.
+template <int MP, int kAct = kActSilu, bool kWK = false, bool kStoreGU = false>
 __global__ void __launch_bounds__(kSmallThreads, SmallCfg<MP>::kCtasPerSm)
 smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                      const __grid_constant__ CUtensorMap tmap_w1,
@@ -108,6 +114,10 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   };
 
   if (threadIdx.x == 0) SWIGLU_TRACE_POINT(0);
+  const bool clk_probe = p.clk != nullptr && blockIdx.x == 0 && threadIdx.x == 0;
+  long long clk_c0 = 0;
+  uint64_t clk_t0 = 0;
+  if (clk_probe) { clk_c0 = clock64(); clk_t0 = globaltimer_ns(); }
   // ------------------------------------------------------------------ setup
   if (warp == 0) {
     if (lane == 0) {
@@ -261,9 +271,16 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
         }
       }
       if (n < p.N) {  // N % 8 == 0 and n % 4 == 0: the 4 columns are in range together
-        const uint32_t lo = pack_bf16x2_rn(glu_mul<kAct>(gs.x, us.x), glu_mul<kAct>(gs.y, us.y));
-        const uint32_t hi = pack_bf16x2_rn(glu_mul<kAct>(gs.z, us.z), glu_mul<kAct>(gs.w, us.w));
-        *reinterpret_cast<uint2*>(Y + (long long)m * p.ldy + n) = make_uint2(lo, hi);
+        if constexpr (kStoreGU) {
+          *reinterpret_cast<uint2*>(Y + (long long)m * p.ldy + n) =
+              make_uint2(pack_bf16x2_rn(gs.x, gs.y), pack_bf16x2_rn(gs.z, gs.w));
+          *reinterpret_cast<uint2*>(p.U + (long long)m * p.ldy + n) =
+              make_uint2(pack_bf16x2_rn(us.x, us.y), pack_bf16x2_rn(us.z, us.w));
+        } else {
+          const uint32_t lo = pack_bf16x2_rn(glu_mul<kAct>(gs.x, us.x), glu_mul<kAct>(gs.y, us.y));
+          const uint32_t hi = pack_bf16x2_rn(glu_mul<kAct>(gs.z, us.z), glu_mul<kAct>(gs.w, us.w));
+          *reinterpret_cast<uint2*>(Y + (long long)m * p.ldy + n) = make_uint2(lo, hi);
+        }
       }
     }
   }
@@ -279,6 +296,10 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     tmem_dealloc<1>(tmem_base, Cfg::kTmemCols);
   }
   if (threadIdx.x == 0) SWIGLU_TRACE_POINT(8);
+  if (clk_probe) {
+    p.clk[0] = (unsigned long long)(clock64() - clk_c0);
+    p.clk[1] = globaltimer_ns() - clk_t0;
+  }
 }
 
 }  // namespace swiglu

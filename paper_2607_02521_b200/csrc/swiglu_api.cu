@@ -6,6 +6,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
+#include <atomic>
 #include <cstring>
 #include <map>
 #include <mutex>
@@ -39,6 +40,10 @@ int fail_cuda(cudaError_t e, const char* what) {
 #ifdef SWIGLU_TRACE
 unsigned long long* g_trace = nullptr;  // debug builds: device buffer for globaltimer stamps
 #endif
+// swiglu_set_clock_probe: device buffer of two uint64 that CTA 0 of every GEMM-class launch
+// fills with {SM cycles, nanoseconds} from entry to exit (measurement aid: the SM clock the
+// kernel actually ran at = cycles / ns).  NULL = off.
+std::atomic<unsigned long long*> g_clk{nullptr};
 
 // ------------------------------------------------------------------ variant tables
 enum FusedVariant {
@@ -48,21 +53,58 @@ enum FusedVariant {
   kFused1CtaN64 = 3,  // 128x64 (Gate|Up) tile per CTA: twice the tiles when N/128 < #SMs
   kNumFused = 4
 };
-enum UnfusedVariant { kUnfused1Cta = 0, kUnfused2Cta = 1, kNumUnfused = 2 };
+enum UnfusedVariant {
+  kUnfused1Cta = 0,    // GEMM 128x256 tiles x2 + elementwise
+  kUnfused2Cta = 1,    // GEMM 256x256 pair tiles x2 + elementwise
+  kUnfusedSmallM = 2,  // M <= 128: ONE merged Gate|Up swap-AB split-K GEMM + elementwise
+  kNumUnfused = 3
+};
 const char* const kFusedNames[kNumFused] = {"fused_1cta_128x128", "fused_2cta_256x128",
                                             "fused_smallm_swapab_splitk", "fused_1cta_128x64"};
 const char* const kUnfusedNames[kNumUnfused] = {"unfused_1cta_gemm128x256+silu_mul",
-                                                "unfused_2cta_gemm256x256+silu_mul"};
+                                                "unfused_2cta_gemm256x256+silu_mul",
+                                                "unfused_smallm_gateup_gemm+silu_mul"};
 
 int env_int(const char* name, int dflt) {
   const char* v = getenv(name);
   return (v && *v) ? atoi(v) : dflt;
 }
 
+// Experiment / A-B overrides.  Read from the environment ONCE, at the
+// first call into the library (and again only on swiglu_reload_env()): the hot path does no
+// getenv.  All default to "off" / "automatic".
+struct Env {
+  int variant = -1, unfused_variant = -1, ksplit = 0, group_m = 0, host_chunks = 4;
+  bool no_pdl = false, no_prefetch = false, no_early = false, no_tail_split = false,
+       no_w_evict_first = false, no_tmap_cache = false;
+};
+Env g_env;
+std::once_flag g_env_once;
+void load_env() {
+  Env e;
+  e.variant = env_int("SWIGLU_VARIANT", -1);
+  e.unfused_variant = env_int("SWIGLU_UNFUSED_VARIANT", -1);
+  e.ksplit = env_int("SWIGLU_KSPLIT", 0);
+  e.group_m = env_int("SWIGLU_GROUP_M", 0);
+  e.host_chunks = env_int("SWIGLU_HOST_CHUNKS", 4);
+  if (e.host_chunks <= 0) e.host_chunks = 4;
+  e.no_pdl = env_int("SWIGLU_NO_PDL", 0) != 0;
+  e.no_prefetch = env_int("SWIGLU_NO_PREFETCH", 0) != 0;
+  e.no_early = env_int("SWIGLU_NO_EARLY", 0) != 0;
+  e.no_tail_split = env_int("SWIGLU_NO_TAIL_SPLIT", 0) != 0;
+  e.no_w_evict_first = env_int("SWIGLU_NO_W_EVICT_FIRST", 0) != 0;
+  e.no_tmap_cache = env_int("SWIGLU_NO_TMAP_CACHE", 0) != 0;
+  g_env = e;
+}
+const Env& env() {
+  std::call_once(g_env_once, load_env);
+  return g_env;
+}
+
 // Measured dispatch (table regenerated from bench sweeps).
 int select_fused(int64_t M, int64_t N, int64_t K) {
   (void)K;
-  const int forced = env_int("SWIGLU_VARIANT", -1);
+  const int forced = env().variant;
   if (forced >= 0 && forced < kNumFused) {
     if (forced != kFusedSmallM || M <= swiglu::kSmallMMax) return forced;
   }
@@ -82,9 +124,12 @@ int select_fused(int64_t M, int64_t N, int64_t K) {
 }
 int select_unfused(int64_t M, int64_t N, int64_t K) {
   (void)N; (void)K;
-  const int forced = env_int("SWIGLU_UNFUSED_VARIANT", -1);
-  if (forced >= 0 && forced < kNumUnfused) return forced;
-  return (M <= 128) ? kUnfused1Cta : kUnfused2Cta;
+  const int forced = env().unfused_variant;
+  if (forced >= 0 && forced < kNumUnfused && (forced != kUnfusedSmallM || M <= swiglu::kSmallMMax))
+    return forced;
+  // Decode sizes: the same swap-AB split-K streaming kernel as the fused path, writing bf16
+  // Gate and Up -- so that fused vs unfused compares fusion, not tile shapes.
+  return (M <= 128) ? kUnfusedSmallM : kUnfused2Cta;
 }
 
 // ------------------------------------------------------------------ validation (no CUDA)
@@ -130,7 +175,9 @@ struct DeviceState {
   struct Buf { void* ptr = nullptr; size_t bytes = 0; };
   std::map<cudaStream_t, Buf> workspace;     // unfused path: bf16 Gate | Up
   std::map<cudaStream_t, Buf> host_scratch;  // swiglu_mlp_host: device copies of A, W1, W2, Y
-  // swiglu_mlp_host_batched: copy streams and events of its H2D / compute / D2H pipeline
+  // swiglu_mlp_host_batched: copy streams and events of its H2D / compute / D2H pipeline;
+  // host_mu admits one such pipeline per device at a time
+  std::mutex host_mu;
   cudaStream_t s_in = nullptr, s_out = nullptr;
   cudaEvent_t ev_a = nullptr, ev_in[2] = {nullptr, nullptr}, ev_cmp[2] = {nullptr, nullptr},
               ev_out[2] = {nullptr, nullptr};
@@ -156,7 +203,11 @@ int set_smem_attrs() {
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kAct, kWK>, attr, SmallCfg<32>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kAct, kWK>, attr, SmallCfg<64>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<128, kAct, kWK>, attr, SmallCfg<128>::kSmemBytes));
-  if (kAct == kActSilu) {  // the unfused path's plain GEMM has no activation
+  if (kAct == kActSilu) {  // the unfused path's plain GEMMs have no activation
+    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kActSilu, kWK, true>, attr, SmallCfg<16>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kActSilu, kWK, true>, attr, SmallCfg<32>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kActSilu, kWK, true>, attr, SmallCfg<64>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<128, kActSilu, kWK, true>, attr, SmallCfg<128>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, false, 128, kActSilu, kWK>, attr, GemmCfg<1>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, false, 128, kActSilu, kWK>, attr, GemmCfg<2>::kSmemBytes));
   }
@@ -199,10 +250,50 @@ int get_device_state(DeviceState** out) {
   return SWIGLU_OK;
 }
 
+// Tensor-map cache (a0: "build or fetch cached CUtensorMaps").  A map is a pure function of
+// (base, inner, outer, box): a cached copy can never be stale, whatever happened to the
+// allocation in between.  Thread-local and direct-mapped, so the hot path takes no lock.
+struct TmapKey {
+  const void* base; int64_t inner, outer; uint32_t box_inner, box_outer;
+  bool operator==(const TmapKey& o) const {
+    return base == o.base && inner == o.inner && outer == o.outer && box_inner == o.box_inner &&
+           box_outer == o.box_outer;
+  }
+};
+struct TmapSlot { bool used = false; TmapKey key; CUtensorMap map; };
+constexpr int kTmapSlots = 256;
+thread_local TmapSlot t_tmaps[kTmapSlots];
+thread_local uint64_t t_tmap_hits = 0, t_tmap_misses = 0;
+
+int encode_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
+                uint32_t box_inner, uint32_t box_outer);
+
 // 2-D bf16 row-major tensor [outer, inner] (inner contiguous), box = box_outer x box_inner,
 // 128-byte swizzle (box_inner must be 64 elements), out-of-bounds reads give zeros.
 int make_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
               uint32_t box_inner, uint32_t box_outer) {
+  if (env().no_tmap_cache) return encode_tmap(out, base, inner, outer, box_inner, box_outer);
+  const TmapKey key{base, inner, outer, box_inner, box_outer};
+  uint64_t h = (uint64_t)(uintptr_t)base * 0x9E3779B97F4A7C15ull;
+  h ^= ((uint64_t)inner * 0xC2B2AE3D27D4EB4Full) ^ ((uint64_t)outer * 0x165667B19E3779F9ull) ^
+       ((uint64_t)box_outer << 7) ^ box_inner;
+  TmapSlot& slot = t_tmaps[(h >> 40) & (kTmapSlots - 1)];
+  if (slot.used && slot.key == key) {
+    ++t_tmap_hits;
+    *out = slot.map;
+    return SWIGLU_OK;
+  }
+  ++t_tmap_misses;
+  const int rc = encode_tmap(out, base, inner, outer, box_inner, box_outer);
+  if (rc) return rc;
+  slot.used = true;
+  slot.key = key;
+  slot.map = *out;
+  return SWIGLU_OK;
+}
+
+int encode_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
+                uint32_t box_inner, uint32_t box_outer) {
   const cuuint64_t dims[2] = {(cuuint64_t)inner, (cuuint64_t)outer};
   const cuuint64_t strides[1] = {(cuuint64_t)inner * 2};
   const cuuint32_t box[2] = {box_inner, box_outer};
@@ -217,10 +308,7 @@ int make_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
   return SWIGLU_OK;
 }
 
-bool pdl_enabled() {
-  static const bool on = env_int("SWIGLU_NO_PDL", 0) == 0;
-  return on;
-}
+bool pdl_enabled() { return !env().no_pdl; }
 
 // ------------------------------------------------------------------ launches
 template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = swiglu::kActSilu, bool kWK = false>
@@ -243,7 +331,7 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   p.n_tiles = (int)((N + out_cols - 1) / out_cols);
   // L2 raster group: keep the slab of A the running CTAs share at <= 32 MiB
   int64_t gm = (32ll << 20) / ((int64_t)rows_per_tile * K * 2);
-  const int forced_gm = env_int("SWIGLU_GROUP_M", 0);
+  const int forced_gm = env().group_m;
   if (forced_gm > 0) gm = forced_gm;
   if (gm < 1) gm = 1;
   if (gm > p.m_tiles) gm = p.m_tiles;
@@ -255,7 +343,7 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   // 64-column halves so the wave takes half a tile time on all SMs (fused 128-column tiles only).
   p.wide_tiles = (int)tiles;
   p.total_tiles = (int)tiles;
-  if (kFused && kBN == 128 && tiles > groups && !env_int("SWIGLU_NO_TAIL_SPLIT", 0)) {
+  if (kFused && kBN == 128 && tiles > groups && !env().no_tail_split) {
     const int64_t rem = tiles % groups;
     if (rem > 0 && 2 * rem <= groups) {
       p.wide_tiles = (int)(tiles - rem);
@@ -263,8 +351,9 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
     }
   }
   // one tile per CTA (a short, HBM-bound call): fill the TMA ring before the setup barrier
-  p.early_issue = (kCtaGroup == 1 && kFused && tiles <= groups && !env_int("SWIGLU_NO_EARLY", 0));
-  p.w_evict_first = (p.m_tiles == 1 && !env_int("SWIGLU_NO_W_EVICT_FIRST", 0));
+  p.early_issue = (kCtaGroup == 1 && kFused && tiles <= groups && !env().no_early);
+  p.w_evict_first = (p.m_tiles == 1 && !env().no_w_evict_first);
+  p.clk = g_clk.load(std::memory_order_relaxed);
 #ifdef SWIGLU_TRACE
   p.trace = g_trace;
 #endif
@@ -304,7 +393,7 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
 //    cluster (clusters of 5-8 do not all fit at once and run in a second wave) and never fewer
 //    than 4 k-blocks per CTA (the cluster barrier + DSMEM reduction cost grows with S).
 int smallm_ksplit(int sm_count, int ctas_per_sm, int mp, int64_t n_tiles, int64_t k_blocks) {
-  const int forced = env_int("SWIGLU_KSPLIT", 0);
+  const int forced = env().ksplit;
   const int64_t slots = (int64_t)ctas_per_sm * sm_count;
   int64_t s;
   if (n_tiles >= sm_count) {
@@ -321,9 +410,9 @@ int smallm_ksplit(int sm_count, int ctas_per_sm, int mp, int64_t n_tiles, int64_
   return (int)s;
 }
 
-template <int MP, int kAct, bool kWK>
+template <int MP, int kAct, bool kWK, bool kStoreGU = false>
 int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const void* W2,
-                     void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
+                     void* Y, void* U, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
   using namespace swiglu;
   CUtensorMap ta, tw1, tw2;
   int rc;
@@ -335,11 +424,13 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   p.M = (int)M; p.N = (int)N; p.K = (int)K;
   p.ksplit = smallm_ksplit(d.sm_count, SmallCfg<MP>::kCtasPerSm, MP, n_tiles, k_blocks);
   p.ldy = N;
+  p.U = (uint16_t*)U;
+  p.clk = g_clk.load(std::memory_order_relaxed);
   // L2 prefetch ahead of the grid dependency: at most ~32 MiB over the whole grid
   const int64_t grid = n_tiles * p.ksplit;
   int64_t pf = (32ll << 20) / (grid * 2 * SmallCfg<MP>::kWBytes);
   if (pf > kSmallPrefetchMax) pf = kSmallPrefetchMax;
-  if (env_int("SWIGLU_NO_PREFETCH", 0)) pf = 0;
+  if (env().no_prefetch) pf = 0;
   p.prefetch_blocks = (int)pf;
 #ifdef SWIGLU_TRACE
   p.trace = g_trace;
@@ -366,18 +457,18 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   }
   cfg.attrs = attrs;
   cfg.numAttrs = na;
-  CUDA_TRY(cudaLaunchKernelEx(&cfg, smallm_swiglu_kernel<MP, kAct, kWK>, ta, tw1, tw2, (uint16_t*)Y,
-                              p));
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, smallm_swiglu_kernel<MP, kAct, kWK, kStoreGU>, ta, tw1, tw2,
+                              (uint16_t*)Y, p));
   return SWIGLU_OK;
 }
 
-template <int kAct, bool kWK>
+template <int kAct, bool kWK, bool kStoreGU = false>
 int launch_smallm(const DeviceState& d, const void* A, const void* W1, const void* W2, void* Y,
-                  int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
-  if (M <= 16) return launch_smallm_mp<16, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
-  if (M <= 32) return launch_smallm_mp<32, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
-  if (M <= 64) return launch_smallm_mp<64, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
-  return launch_smallm_mp<128, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
+                  void* U, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
+  if (M <= 16) return launch_smallm_mp<16, kAct, kWK, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream);
+  if (M <= 32) return launch_smallm_mp<32, kAct, kWK, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream);
+  if (M <= 64) return launch_smallm_mp<64, kAct, kWK, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream);
+  return launch_smallm_mp<128, kAct, kWK, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream);
 }
 
 template <int kAct>
@@ -428,29 +519,47 @@ size_t workspace_for(int64_t M, int64_t N, int64_t K, int unfused, int variant) 
   return 0;  // fused variants reduce split-K partials on chip (DSMEM), no global workspace
 }
 
-// Grow-only buffer of `stream` in `pool`.  Growing waits for that stream's earlier work (which
-// may still be using the old buffer) and allocates; never while the stream is capturing.
+// Library-owned buffer of `stream` in `pool`, at least `need` bytes.  Allocation and growth are
+// STREAM-ORDERED (cudaMallocAsync / cudaFreeAsync on `stream`): the old block is released only
+// after the work already enqueued on `stream` that may still use it, and nothing here
+// synchronises.  Never under stream capture: a captured graph would keep a pointer the next
+// growth frees, so capture needs the _ex form with a caller workspace (include/swiglu_mlp.h).
 int ensure_stream_buffer(std::map<cudaStream_t, DeviceState::Buf>& pool, size_t need,
                          cudaStream_t stream, void** out) {
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(stream, &cap);
+  if (cap != cudaStreamCaptureStatusNone)
+    return fail(SWIGLU_ERR_WORKSPACE,
+                "the library-owned workspace (%zu bytes) cannot be used while the stream is "
+                "capturing; use the _ex form with a caller workspace", need);
   std::lock_guard<std::mutex> lk(g_mu);
   DeviceState::Buf& b = pool[stream];
   if (need > b.bytes) {
-    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-    cudaStreamIsCapturing(stream, &cap);
-    if (cap != cudaStreamCaptureStatusNone)
-      return fail(SWIGLU_ERR_WORKSPACE,
-                  "library workspace must grow to %zu bytes but the stream is capturing; "
-                  "use the _ex form with a caller workspace", need);
     if (b.ptr) {
-      CUDA_TRY(cudaStreamSynchronize(stream));
-      CUDA_TRY(cudaFree(b.ptr));
+      CUDA_TRY(cudaFreeAsync(b.ptr, stream));
       b.ptr = nullptr;
       b.bytes = 0;
     }
-    CUDA_TRY(cudaMalloc(&b.ptr, need));
+    CUDA_TRY(cudaMallocAsync(&b.ptr, need, stream));
     b.bytes = need;
   }
   *out = b.ptr;
+  return SWIGLU_OK;
+}
+
+// Return every library-owned buffer of `pool` that belongs to `stream` (or to any stream).
+int release_pool(std::map<cudaStream_t, DeviceState::Buf>& pool, bool all, cudaStream_t stream) {
+  for (auto it = pool.begin(); it != pool.end();) {
+    if (all || it->first == stream) {
+      if (it->second.ptr) {
+        if (all) CUDA_TRY(cudaFree(it->second.ptr));  // the caller has synchronised the device
+        else CUDA_TRY(cudaFreeAsync(it->second.ptr, stream));
+      }
+      it = pool.erase(it);
+    } else {
+      ++it;
+    }
+  }
   return SWIGLU_OK;
 }
 
@@ -460,7 +569,7 @@ int launch_fused_l(const DeviceState& d, int variant, const void* A, const void*
   switch (variant) {
     case kFused1Cta: return launch_gemm<1, true, 128, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
     case kFused2Cta: return launch_gemm<2, true, 128, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
-    case kFusedSmallM: return launch_smallm<kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
+    case kFusedSmallM: return launch_smallm<kAct, kWK>(d, A, W1, W2, Y, nullptr, M, N, K, stream);
     case kFused1CtaN64: return launch_gemm<1, true, 64, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
   }
   return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
@@ -510,6 +619,9 @@ int run_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t 
     return fail(SWIGLU_ERR_UNSUPPORTED, "unknown activation %d", act);
   if (variant < -1 || variant >= kNumUnfused)
     return fail(SWIGLU_ERR_UNSUPPORTED, "unknown unfused variant %d", variant);
+  if (variant == kUnfusedSmallM && M > swiglu::kSmallMMax)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "variant %s handles M <= %d only",
+                kUnfusedNames[kUnfusedSmallM], swiglu::kSmallMMax);
   if (M == 0) return SWIGLU_OK;
   const size_t need = workspace_for(M, N, K, 1, variant);
   if (!own_ws) {
@@ -523,7 +635,11 @@ int run_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t 
   void* G = ws;
   void* U = (char*)ws + need / 2;
   using swiglu::kActSilu;
-  if (variant == kUnfused1Cta && !layout) {
+  if (variant == kUnfusedSmallM) {
+    rc = layout ? launch_smallm<kActSilu, true, true>(*d, A, W1, W2, G, U, M, N, K, stream)
+                : launch_smallm<kActSilu, false, true>(*d, A, W1, W2, G, U, M, N, K, stream);
+    if (rc) return rc;
+  } else if (variant == kUnfused1Cta && !layout) {
     if ((rc = launch_gemm<1, false>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
     if ((rc = launch_gemm<1, false>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
   } else if (variant == kUnfused1Cta) {
@@ -646,9 +762,10 @@ int swiglu_selected_variant(int64_t M, int64_t N, int64_t K, int unfused) {
 }
 
 int swiglu_launches_per_call(int64_t M, int64_t N, int64_t K, int unfused, int variant) {
-  (void)N; (void)K; (void)variant;
   if (M <= 0) return 0;
-  return unfused ? 3 : 1;
+  if (!unfused) return 1;
+  if (variant < 0) variant = select_unfused(M, N, K);
+  return variant == kUnfusedSmallM ? 2 : 3;  // merged Gate|Up GEMM, or two GEMMs; + elementwise
 }
 
 int swiglu_mlp_host(const void* A_host, const void* W1_host, const void* W2_host, void* Y_host,
@@ -707,9 +824,8 @@ int swiglu_mlp_host_batched(const void* const* A_host, void* const* Y_host, cons
   cudaStreamIsCapturing(stream, &cap);
   if (cap != cudaStreamCaptureStatusNone)
     return fail(SWIGLU_ERR_UNSUPPORTED, "the host-buffer forms synchronise; not capturable");
-  // One pipeline per device at a time (it owns the copy streams and events below).
-  static std::mutex host_mu;
-  std::lock_guard<std::mutex> host_lk(host_mu);
+  // One pipeline per DEVICE at a time (it owns that device's copy streams and events).
+  std::lock_guard<std::mutex> host_lk(d->host_mu);
   if (!d->s_in) {
     CUDA_TRY(cudaStreamCreateWithFlags(&d->s_in, cudaStreamNonBlocking));
     CUDA_TRY(cudaStreamCreateWithFlags(&d->s_out, cudaStreamNonBlocking));
@@ -722,26 +838,33 @@ int swiglu_mlp_host_batched(const void* const* A_host, void* const* Y_host, cons
   }
   // Column chunks of the weights: H2D of chunk j+1 and D2H of chunk j-1 run under the kernels
   // of chunk j (the path has no dependency between output columns).
-  const int want_chunks = env_int("SWIGLU_HOST_CHUNKS", 4) > 0 ? env_int("SWIGLU_HOST_CHUNKS", 4) : 4;
+  const int want_chunks = env().host_chunks;
   int64_t nc = round_up((size_t)((N + want_chunks - 1) / want_chunks), 128);
   if (nc < 512) nc = 512;
   if (nc > N) nc = N;
   const int chunks = (int)((N + nc - 1) / nc);
   const size_t a_bytes = round_up((size_t)rows * K * 2, 256);
   const size_t w_bytes = round_up((size_t)K * nc * 2, 256);
-  const size_t y_bytes = round_up((size_t)rows * nc * 2, 256);
+  // One Y buffer holds every batch's [M[i], nc] block, each block padded to 256 bytes.
+  size_t y_bytes = 0;
+  for (int i = 0; i < count; ++i)
+    if (M[i] > 0) y_bytes += round_up((size_t)M[i] * nc * 2, 256);
   void* scratch;
   if ((rc = ensure_stream_buffer(d->host_scratch, a_bytes + 4 * w_bytes + 2 * y_bytes, stream,
                                  &scratch)))
     return rc;
   char* dA = (char*)scratch;
   char* dW = dA + a_bytes;                // [2 buffers][W1c | W2c]
-  char* dY = dW + 4 * w_bytes;            // [2 buffers][rows x nc]
-  // everything the caller enqueued on `stream` so far comes first
-  CUDA_TRY(cudaEventRecord(d->ev_a, stream));
-  CUDA_TRY(cudaStreamWaitEvent(d->s_in, d->ev_a, 0));
-  CUDA_TRY(cudaStreamWaitEvent(d->s_out, d->ev_a, 0));
-  {
+  char* dY = dW + 4 * w_bytes;            // [2 buffers][sum_i pad256(M[i] x nc)]
+
+  // The enqueue phase.  On ANY failure the copies and kernels already enqueued still reference
+  // the library's scratch and the caller's host buffers: drain all three streams before
+  // returning the error, so the caller may free its buffers as soon as the call is back.
+  auto enqueue = [&]() -> int {
+    // everything the caller enqueued on `stream` so far comes first
+    CUDA_TRY(cudaEventRecord(d->ev_a, stream));
+    CUDA_TRY(cudaStreamWaitEvent(d->s_in, d->ev_a, 0));
+    CUDA_TRY(cudaStreamWaitEvent(d->s_out, d->ev_a, 0));
     size_t off = 0;
     for (int i = 0; i < count; ++i) {
       if (M[i] == 0) continue;
@@ -749,48 +872,107 @@ int swiglu_mlp_host_batched(const void* const* A_host, void* const* Y_host, cons
                                d->s_in));
       off += (size_t)M[i] * K * 2;
     }
-  }
-  for (int j = 0; j < chunks; ++j) {
-    const int b = j & 1;
-    const int64_t n0 = (int64_t)j * nc, ncj = (n0 + nc <= N) ? nc : N - n0;
-    char* w1c = dW + (size_t)b * 2 * w_bytes;
-    char* w2c = w1c + w_bytes;
-    char* yc = dY + (size_t)b * y_bytes;
-    // H2D: the weight columns [n0, n0 + ncj), packed dense [K, ncj]
-    if (j >= 2) CUDA_TRY(cudaStreamWaitEvent(d->s_in, d->ev_cmp[b], 0));  // buffer b consumed
-    CUDA_TRY(cudaMemcpy2DAsync(w1c, (size_t)ncj * 2, (const char*)W1_host + n0 * 2, (size_t)N * 2,
-                               (size_t)ncj * 2, (size_t)K, cudaMemcpyHostToDevice, d->s_in));
-    CUDA_TRY(cudaMemcpy2DAsync(w2c, (size_t)ncj * 2, (const char*)W2_host + n0 * 2, (size_t)N * 2,
-                               (size_t)ncj * 2, (size_t)K, cudaMemcpyHostToDevice, d->s_in));
-    CUDA_TRY(cudaEventRecord(d->ev_in[b], d->s_in));
-    // compute on the caller's stream
-    CUDA_TRY(cudaStreamWaitEvent(stream, d->ev_in[b], 0));
-    if (j >= 2) CUDA_TRY(cudaStreamWaitEvent(stream, d->ev_out[b], 0));  // Y buffer b drained
-    size_t a_off = 0, y_off = 0;
-    for (int i = 0; i < count; ++i) {
-      if (M[i] == 0) continue;
-      rc = unfused ? swiglu_mlp_unfused(dA + a_off, w1c, w2c, yc + y_off, M[i], ncj, K, stream_v)
-                   : swiglu_mlp(dA + a_off, w1c, w2c, yc + y_off, M[i], ncj, K, stream_v);
-      if (rc) return rc;
-      a_off += (size_t)M[i] * K * 2;
-      y_off += round_up((size_t)M[i] * ncj * 2, 256);
+    for (int j = 0; j < chunks; ++j) {
+      const int b = j & 1;
+      const int64_t n0 = (int64_t)j * nc, ncj = (n0 + nc <= N) ? nc : N - n0;
+      char* w1c = dW + (size_t)b * 2 * w_bytes;
+      char* w2c = w1c + w_bytes;
+      char* yc = dY + (size_t)b * y_bytes;
+      // H2D: the weight columns [n0, n0 + ncj), packed dense [K, ncj]
+      if (j >= 2) CUDA_TRY(cudaStreamWaitEvent(d->s_in, d->ev_cmp[b], 0));  // buffer b consumed
+      CUDA_TRY(cudaMemcpy2DAsync(w1c, (size_t)ncj * 2, (const char*)W1_host + n0 * 2,
+                                 (size_t)N * 2, (size_t)ncj * 2, (size_t)K,
+                                 cudaMemcpyHostToDevice, d->s_in));
+      CUDA_TRY(cudaMemcpy2DAsync(w2c, (size_t)ncj * 2, (const char*)W2_host + n0 * 2,
+                                 (size_t)N * 2, (size_t)ncj * 2, (size_t)K,
+                                 cudaMemcpyHostToDevice, d->s_in));
+      CUDA_TRY(cudaEventRecord(d->ev_in[b], d->s_in));
+      // compute on the caller's stream
+      CUDA_TRY(cudaStreamWaitEvent(stream, d->ev_in[b], 0));
+      if (j >= 2) CUDA_TRY(cudaStreamWaitEvent(stream, d->ev_out[b], 0));  // Y buffer b drained
+      size_t a_off = 0, y_off = 0;
+      for (int i = 0; i < count; ++i) {
+        if (M[i] == 0) continue;
+        const int r = unfused
+                          ? swiglu_mlp_unfused(dA + a_off, w1c, w2c, yc + y_off, M[i], ncj, K, stream_v)
+                          : swiglu_mlp(dA + a_off, w1c, w2c, yc + y_off, M[i], ncj, K, stream_v);
+        if (r) return r;
+        a_off += (size_t)M[i] * K * 2;
+        y_off += round_up((size_t)M[i] * nc * 2, 256);
+      }
+      CUDA_TRY(cudaEventRecord(d->ev_cmp[b], stream));
+      // D2H: scatter the chunk's columns into each batch's Y
+      CUDA_TRY(cudaStreamWaitEvent(d->s_out, d->ev_cmp[b], 0));
+      y_off = 0;
+      for (int i = 0; i < count; ++i) {
+        if (M[i] == 0) continue;
+        CUDA_TRY(cudaMemcpy2DAsync((char*)Y_host[i] + n0 * 2, (size_t)N * 2, yc + y_off,
+                                   (size_t)ncj * 2, (size_t)ncj * 2, (size_t)M[i],
+                                   cudaMemcpyDeviceToHost, d->s_out));
+        y_off += round_up((size_t)M[i] * nc * 2, 256);
+      }
+      CUDA_TRY(cudaEventRecord(d->ev_out[b], d->s_out));
     }
-    CUDA_TRY(cudaEventRecord(d->ev_cmp[b], stream));
-    // D2H: scatter the chunk's columns into each batch's Y
-    CUDA_TRY(cudaStreamWaitEvent(d->s_out, d->ev_cmp[b], 0));
-    y_off = 0;
-    for (int i = 0; i < count; ++i) {
-      if (M[i] == 0) continue;
-      CUDA_TRY(cudaMemcpy2DAsync((char*)Y_host[i] + n0 * 2, (size_t)N * 2, yc + y_off,
-                                 (size_t)ncj * 2, (size_t)ncj * 2, (size_t)M[i],
-                                 cudaMemcpyDeviceToHost, d->s_out));
-      y_off += round_up((size_t)M[i] * ncj * 2, 256);
-    }
-    CUDA_TRY(cudaEventRecord(d->ev_out[b], d->s_out));
-  }
-  CUDA_TRY(cudaStreamSynchronize(d->s_out));
-  CUDA_TRY(cudaStreamSynchronize(stream));
+    return SWIGLU_OK;
+  };
+  rc = enqueue();
+  const cudaError_t e_in = cudaStreamSynchronize(d->s_in);
+  const cudaError_t e_out = cudaStreamSynchronize(d->s_out);
+  const cudaError_t e_cmp = cudaStreamSynchronize(stream);
+  if (rc) return rc;  // g_err holds the enqueue failure
+  if (e_in != cudaSuccess) return fail_cuda(e_in, "cudaStreamSynchronize(copy-in stream)");
+  if (e_out != cudaSuccess) return fail_cuda(e_out, "cudaStreamSynchronize(copy-out stream)");
+  if (e_cmp != cudaSuccess) return fail_cuda(e_cmp, "cudaStreamSynchronize(stream)");
   return SWIGLU_OK;
+}
+
+int swiglu_release_stream(void* stream_v) {
+  cudaStream_t stream = (cudaStream_t)stream_v;
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return fail(SWIGLU_ERR_CUDA, "device index %d out of range", dev);
+  std::lock_guard<std::mutex> lk(g_mu);
+  DeviceState& d = g_dev[dev];
+  int rc;
+  if ((rc = release_pool(d.workspace, false, stream))) return rc;
+  return release_pool(d.host_scratch, false, stream);
+}
+
+int swiglu_release(void) {
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return fail(SWIGLU_ERR_CUDA, "device index %d out of range", dev);
+  CUDA_TRY(cudaDeviceSynchronize());  // nothing of ours may still be running on the buffers
+  DeviceState& d = g_dev[dev];
+  std::lock_guard<std::mutex> host_lk(d.host_mu);  // lock order: host_mu, then g_mu
+  std::lock_guard<std::mutex> lk(g_mu);
+  int rc;
+  if ((rc = release_pool(d.workspace, true, nullptr))) return rc;
+  if ((rc = release_pool(d.host_scratch, true, nullptr))) return rc;
+  if (d.s_in) {
+    cudaStreamDestroy(d.s_in);
+    cudaStreamDestroy(d.s_out);
+    cudaEventDestroy(d.ev_a);
+    for (int b = 0; b < 2; ++b) {
+      cudaEventDestroy(d.ev_in[b]);
+      cudaEventDestroy(d.ev_cmp[b]);
+      cudaEventDestroy(d.ev_out[b]);
+    }
+    d.s_in = d.s_out = nullptr;
+  }
+  return SWIGLU_OK;
+}
+
+void swiglu_reload_env(void) { load_env(); }
+
+void swiglu_set_clock_probe(void* device_u64x2) {
+  g_clk.store((unsigned long long*)device_u64x2, std::memory_order_relaxed);
+}
+
+int swiglu_tensor_map_cache_stats(uint64_t* hits, uint64_t* misses) {
+  if (hits) *hits = t_tmap_hits;
+  if (misses) *misses = t_tmap_misses;
+  return kTmapSlots;
 }
 
 #ifdef SWIGLU_TRACE

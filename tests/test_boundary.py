@@ -39,7 +39,10 @@ def test_version_status_strings_and_variant_table(lib):
     large = B.swiglu_variant_name(B.swiglu_selected_variant(4096, 8960, 1536))
     assert "smallm" in small and "smallm" not in large
     assert B.swiglu_launches_per_call(16, 4864, 896) == 1
-    assert B.swiglu_launches_per_call(16, 4864, 896, unfused=True) == 3
+    assert B.swiglu_launches_per_call(16, 4864, 896, unfused=True) == 2     # merged Gate|Up GEMM
+    assert B.swiglu_launches_per_call(4096, 8960, 1536, unfused=True) == 3  # two GEMMs + elementwise
+    assert "smallm" in B.swiglu_variant_name(B.swiglu_selected_variant(16, 4864, 896, unfused=True),
+                                             unfused=True)
     assert B.swiglu_launches_per_call(0, 4864, 896) == 0
 
 
@@ -52,6 +55,24 @@ def test_activation_table(lib):
     rc = lib.swiglu_glu_mlp(0x10000000, 0x20000000, 0x30000000, 0x40000000, 4, 16, 8, 7, None)
     assert rc == B.SWIGLU_ERR_UNSUPPORTED            # unknown activation
     assert lib.swiglu_act_mul(0x10, 0x20, 0x30, 16, 5, None) == B.SWIGLU_ERR_UNSUPPORTED
+
+
+def test_env_overrides_are_read_once_and_on_reload(lib, monkeypatch):
+    """The hot path does no getenv: an override set after the first call is invisible until
+    swiglu_reload_env()."""
+    auto = B.swiglu_selected_variant(4096, 8960, 1536)
+    monkeypatch.setenv("SWIGLU_VARIANT", "0")
+    assert B.swiglu_selected_variant(4096, 8960, 1536) == auto      # not re-read
+    B.swiglu_reload_env()
+    assert B.swiglu_selected_variant(4096, 8960, 1536) == 0
+    monkeypatch.delenv("SWIGLU_VARIANT")
+    B.swiglu_reload_env()
+    assert B.swiglu_selected_variant(4096, 8960, 1536) == auto
+
+
+def test_tensor_map_cache_stats_are_callable_without_a_device(lib):
+    hits, misses, slots = B.swiglu_tensor_map_cache_stats()
+    assert slots >= 64 and hits >= 0 and misses >= 0
 
 
 def test_workspace_query(lib):

@@ -26,6 +26,22 @@ def _device():
     yield
 
 
+@pytest.fixture
+def swiglu_env(monkeypatch):
+    """Set SWIGLU_* experiment overrides for one test: the library reads its environment once,
+    so every change is followed by swiglu_reload_env(), and the defaults come back afterwards."""
+    names = []
+
+    def set_(name, value):
+        names.append(name)
+        monkeypatch.setenv(name, str(value))
+        B.swiglu_reload_env()
+    yield set_
+    for n in names:
+        monkeypatch.delenv(n, raising=False)
+    B.swiglu_reload_env()
+
+
 def dev(bits):
     return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).cuda().view(torch.bfloat16)
 
@@ -68,12 +84,14 @@ ODD_SHAPES = [
     (1, 128, 64), (7, 136, 72), (16, 384, 896), (127, 128, 64), (128, 4864, 896),
     (129, 264, 200), (300, 1160, 328), (513, 392, 1096),
 ]
-VARIANTS = [("fused", 0), ("fused", 1), ("fused", 3), ("unfused", 0), ("unfused", 1)]
+VARIANTS = [("fused", 0), ("fused", 1), ("fused", 3), ("unfused", 0), ("unfused", 1), ("unfused", 2)]
 
 
 @pytest.mark.parametrize("kind,variant", VARIANTS)
 @pytest.mark.parametrize("M,N,K", ODD_SHAPES)
 def test_large_m_kernels_on_odd_shapes(kind, variant, M, N, K):
+    if (kind, variant) == ("unfused", 2) and M > 128:
+        pytest.skip("the merged small-M Gate|Up GEMM handles M <= 128")
     A, W1, W2 = inputs.make_case(M, N, K, seed=100 + M + N + K, std=0.05)
     y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
     assert_parity(run(kind, variant, A, W1, W2), y_ref, (kind, variant, M, N, K))
@@ -92,25 +110,27 @@ def test_small_m_kernel_on_odd_shapes(M, N, K):
 
 @pytest.mark.parametrize("ksplit", [1, 2, 3, 5, 8])
 @pytest.mark.parametrize("M", [1, 16, 40, 128])
-def test_small_m_kernel_every_cluster_size(M, ksplit, monkeypatch):
+def test_small_m_kernel_every_cluster_size(M, ksplit, swiglu_env):
     """Forced split-K factor (cluster size): the DSMEM reduction must give the same result
-    for any S, including S that does not divide the number of k-blocks or M."""
-    monkeypatch.setenv("SWIGLU_KSPLIT", str(ksplit))
+    for any S, including S that does not divide the number of k-blocks or M -- in the fused
+    kernel and in the merged Gate|Up GEMM of the unfused path."""
+    swiglu_env("SWIGLU_KSPLIT", ksplit)
     A, W1, W2 = inputs.make_case(M, 520, 712, seed=300 + M, std=0.05)
     y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
     assert_parity(run("fused", 2, A, W1, W2), y_ref, ("smallm", M, ksplit))
+    assert_parity(run("unfused", 2, A, W1, W2), y_ref, ("smallm-unfused", M, ksplit))
 
 
 @pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("M,N,K", [(2560, 1024, 128), (2560, 1032, 72), (2305, 1160, 64)])
-def test_last_wave_half_tiles(variant, M, N, K, monkeypatch):
+def test_last_wave_half_tiles(variant, M, N, K, swiglu_env):
     """Shapes whose tile count leaves a last wave of <= half the CTA groups: those tiles run as
     64-column half tiles (a1).  Same result with the split disabled."""
     A, W1, W2 = inputs.make_case(M, N, K, seed=400 + N + K, std=0.05)
     y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
     y_split = run("fused", variant, A, W1, W2)
     assert_parity(y_split, y_ref, ("tail-split", variant, M, N, K))
-    monkeypatch.setenv("SWIGLU_NO_TAIL_SPLIT", "1")
+    swiglu_env("SWIGLU_NO_TAIL_SPLIT", 1)
     y_plain = run("fused", variant, A, W1, W2)
     assert_parity(y_plain, y_ref, ("no-split", variant, M, N, K))
 
@@ -157,6 +177,51 @@ def test_baseline_full_sizes_sampled_rows(shape):
             rep = check.compare(host(dY[torch.from_numpy(rows).cuda()]), y_ref)
             assert rep.mismatches == 0, (shape, M, entry.__name__, rep)
             del dY
+
+
+@pytest.mark.parametrize("shape", list(inputs.PAPER_SHAPES))
+def test_paper_grid_sampled_rows(shape):
+    """The paper's own grid (Table 1 shapes incl. 14B = 5120 x 13824,
+    M in {256, 512, 1024, 2048, 4096}), automatic dispatch, fused and
+    unfused, 8 rows of EVERY 128-row tile against the oracle."""
+    K, N, seed, Ms = inputs.PAPER_SHAPES[shape]
+    W1, W2 = inputs.make_weights(K, N, seed)
+    A_max = inputs.make_activations(max(Ms), K, seed)
+    dW1, dW2 = dev(W1), dev(W2)
+    budget_rows = 96 if K * N > 10**8 else 256        # oracle cost: ~4NK fp64 FLOP per row
+    for M in Ms:
+        A = A_max[:M]
+        rows = inputs.sample_rows(M)
+        if len(rows) > budget_rows:                   # keep every tile represented
+            rows = rows[np.linspace(0, len(rows) - 1, budget_rows).round().astype(int)]
+        y_ref, _ = oracle.swiglu_oracle_rows(A, W1, W2, rows)
+        dA = dev(A)
+        for entry in (B.swiglu_mlp, B.swiglu_mlp_unfused):
+            dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+            entry(dA, dW1, dW2, dY)
+            torch.cuda.synchronize()
+            assert bool(torch.isfinite(dY.float()).all()), (shape, M, entry.__name__)
+            rep = check.compare(host(dY[torch.from_numpy(rows).cuda()]), y_ref)
+            assert rep.mismatches == 0, (shape, M, entry.__name__, rep)
+            del dY
+
+
+@pytest.mark.parametrize("shape", list(inputs.SHAPES))
+def test_baseline_full_matrix_one_large_m_per_shape(shape):
+    """"Full-matrix checking remains the default".  Every output of one
+    compute-bound point per BASELINE.json shape (M = 1024; 0.5B has only M = 16 in the grid, so
+    it gets an extra M = 1024 batch) against the oracle, automatic dispatch, fused path."""
+    K, N, seed, _ = inputs.SHAPES[shape]
+    M = 1024
+    W1, W2 = inputs.make_weights(K, N, seed)
+    A = inputs.make_activations(M, K, seed)
+    dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+    B.swiglu_mlp(dev(A), dev(W1), dev(W2), dY)
+    torch.cuda.synchronize()
+    y = host(dY)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+    rep = assert_parity(y, y_ref, (shape, "full matrix"))
+    assert rep.checked == M * N
 
 
 ACTS = ["gelu", "gelu_tanh", "relu"]
@@ -301,6 +366,8 @@ def test_no_write_outside_y_or_workspace(M, N, K):
         assert_parity(host(dY), y_ref, ("guarded", variant, M, N, K))
     need = B.swiglu_workspace_bytes(M, N, K, unfused=True)
     for variant in range(B.swiglu_num_variants(True)):
+        if "smallm" in B.swiglu_variant_name(variant, unfused=True) and M > 128:
+            continue
         ybuf, yv = banded(M * N)
         wbuf, wv = banded(need // 2)
         dY = yv.view(torch.bfloat16).view(M, N)
