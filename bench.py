@@ -735,6 +735,56 @@ def run_all(args):
     print(json.dumps({"clocks": clocks, "peak_source": peak_src}))
 
 
+def run_decode_study(args):
+    """Decode-size anatomy (`--decode-study`): per (shape, M <= 128), microseconds per call in a
+    CUDA-graph chain (cold L2, rotating weight copies) of
+      * the launch-floor probe (the decode kernel's launch with an empty body),
+      * swiglu_mlp (plain [K,N] weights),
+      * swiglu_mlp_packed (prepacked W_fused: one TMA box per stage, weight loads ahead of
+        griddepcontrol.wait),
+      * swiglu_mlp_unfused,
+    plus the isolated (device idle before the call) time of the two fused forms.
+    Writes gpurun_out/decode_study.md."""
+    import torch
+    from paper_2607_02521_b200 import binding as B, inputs
+    lib = B.load()
+    peaks, _ = load_peaks()
+    table = list(inputs.SHAPES) + list(inputs.PAPER_SHAPES)
+    names = [n for n in table if n in args.only.split(",")] if args.only else list(inputs.SHAPES)
+    Ms = [int(m) for m in args.sweep_m.split(",") if int(m) <= 128]
+    lines = ["| workload | M | HBM roofline us | floor probe us | fused us | packed us | unfused us | "
+             "fused isolated us | packed isolated us | fused % of roofline | packed % of roofline |",
+             "|" + "---|" * 11]
+    for name in names:
+        wl = Workload(name, Ms=Ms)
+        nbytes = B.swiglu_packed_weight_bytes(wl.N, wl.K)
+        Wp = [torch.empty(nbytes // 2, dtype=torch.int16, device="cuda") for _ in range(wl.copies)]
+        for c in range(wl.copies):
+            B.swiglu_pack_weights(wl.W1[c], wl.W2[c], Wp[c], wl.N, wl.K)
+        torch.cuda.synchronize()
+        ptrs = {wl.W1[c].data_ptr(): Wp[c].data_ptr() for c in range(wl.copies)}
+
+        def packed(a, w1, w2, y, m, n, k, stream):
+            return lib.swiglu_mlp_packed(a, ptrs[w1], y, m, n, k, stream)
+
+        for M in Ms:
+            probe_fn = lib.swiglu_launch_floor_probe
+            res = time_points(wl, [probe_fn, lib.swiglu_mlp, packed, wl.unfused_fn(M)], M,
+                              batches=args.sweep_batches)
+            iso_f = time_isolated(wl, lib.swiglu_mlp, M)
+            iso_p = time_isolated(wl, packed, M)
+            t_roof, _ = roofline_time_s(M, wl.N, wl.K, peaks["bf16_tflops"], peaks["hbm_gbs"])
+            us = [r["us_median"] for r in res]
+            lines.append(f"| {name} | {M} | {t_roof * 1e6:.2f} | {us[0]:.2f} | {us[1]:.2f} | {us[2]:.2f} | "
+                         f"{us[3]:.2f} | {iso_f:.2f} | {iso_p:.2f} | {100 * t_roof * 1e6 / us[1]:.1f} | "
+                         f"{100 * t_roof * 1e6 / us[2]:.1f} |")
+            print(lines[-1], flush=True)
+        del wl, Wp
+        torch.cuda.empty_cache()
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    open(os.path.join(ROOT, "gpurun_out", "decode_study.md"), "w").write("\n".join(lines) + "\n")
+
+
 def run_sweep(args):
     """Dispatch-table sweeps (`--sweep variants` / `--sweep ksplit`): time every fused variant
     (forced through swiglu_mlp_ex) or every split-K factor of the small-M kernel
@@ -819,6 +869,7 @@ def main():
     ap.add_argument("--sweep", default="", choices=["", "variants", "ksplit"])
     ap.add_argument("--sweep-m", default="1,16,32,64,128,256")
     ap.add_argument("--sweep-batches", type=int, default=15)
+    ap.add_argument("--decode-study", action="store_true")
     args = ap.parse_args()
     from paper_2607_02521_b200.dist import Ranks
     if args.impl == "reference":
@@ -834,6 +885,9 @@ def main():
         return
     if args.sweep:
         run_sweep(args)
+        return
+    if args.decode_study:
+        run_decode_study(args)
         return
     ranks = Ranks()
     if ranks.world != args.gpus and ranks.rank == 0:

@@ -135,6 +135,53 @@ int swiglu_glu_mlp_layout(const void* A, const void* W1, const void* W2, void* Y
                           int64_t N, int64_t K, int activation, int weight_layout, int unfused,
                           int variant, void* stream);
 
+/*
+ * Prepacked, tile-interleaved weights (Kernel-2 "interleaves W1
+ * and W2 ... a one-time preprocessing step").  The paper interleaves
+ * single columns for its Epilogue Visitor Tree; the unit that matters on sm_100a is the
+ * 64-column slab (one 128-byte swizzled TMA box row = one UMMA operand atom), so W_fused is
+ *
+ *     Wp[t][s][k][c]   t < ceil(N/128) column tiles, s in {g0, u0, g1, u1}, k < K, c < 64
+ *                    = W1[k][128 t + 64 (s>>1) + c]  for s even (Gate slabs)
+ *                    = W2[k][128 t + 64 (s>>1) + c]  for s odd  (Up slabs)
+ *                    = 0 for columns >= N                         (bf16, dense, slab-major)
+ *
+ * i.e. swiglu_packed_weight_bytes(N, K) = 2 * K * pad128(N) * 2 bytes.  One 3-D TMA box then
+ * brings a whole Gate|Up stage (instead of four boxes from two tensors), every 8 KB slab block is
+ * contiguous in HBM, and the accumulator columns come out as g0 u0 g1 u1.
+ *
+ * swiglu_pack_weights: device pointers; W1, W2 in `weight_layout` (SWIGLU_WEIGHTS_KN or _NK);
+ *   Wp 16-byte aligned (128-byte recommended), not overlapping W1 / W2.  Asynchronous on
+ *   `stream`.  Its time is NOT part of any swiglu_mlp_packed timing (the paper excludes the
+ *   interleave from its timings too, lines 159, 167).
+ * swiglu_mlp_packed / swiglu_glu_mlp_packed: as swiglu_mlp / swiglu_glu_mlp_ex with (W1, W2)
+ *   replaced by Wp.  CONTRACT: a packed buffer is a CONSTANT while calls that read it are in
+ *   flight or being enqueued.  It must have been written by ordinary stream work (a copy, or a
+ *   kernel that does not signal programmatic launch completion before its last write to Wp;
+ *   swiglu_pack_weights is such a kernel), so "pack, then swiglu_mlp_packed on the same stream"
+ *   is safe without a synchronisation.  In exchange the decode kernel issues its weight loads
+ *   BEFORE griddepcontrol.wait: under programmatic dependent launch the weight stream of call
+ *   i+1 overlaps the tail of call i, and only the activation tile waits for the previous kernel.
+ */
+size_t swiglu_packed_weight_bytes(int64_t N, int64_t K); /* 0 for bad N, K */
+int swiglu_pack_weights(const void* W1, const void* W2, void* Wp, int64_t N, int64_t K,
+                        int weight_layout, void* stream);
+int swiglu_mlp_packed(const void* A, const void* Wp, void* Y, int64_t M, int64_t N, int64_t K,
+                      void* stream);
+int swiglu_glu_mlp_packed(const void* A, const void* Wp, void* Y, int64_t M, int64_t N,
+                          int64_t K, int activation, int variant, void* stream);
+
+/*
+ * Launch-floor probe (measurement aid): enqueues the decode kernel that swiglu_mlp would pick
+ * for this (M <= 128, N, K) -- same grid, cluster dimensions, shared memory, tensor-map
+ * parameters, barrier initialisation, TMEM allocation and programmatic-dependent-launch
+ * attribute -- with its body reduced to prologue + griddepcontrol.wait + teardown: no loads, no
+ * MMAs, no reduction, no stores (Y is not written).  Timing a chain of these gives the
+ * launch-to-launch floor of a dependent kernel chain that the real kernel's time sits on.
+ */
+int swiglu_launch_floor_probe(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                              int64_t N, int64_t K, void* stream);
+
 /* Elementwise stage with a chosen activation: Y[i] = bf16(act(G[i]) * U[i]); see swiglu_silu_mul. */
 int swiglu_act_mul(const void* G, const void* U, void* Y, int64_t elems, int activation,
                    void* stream);

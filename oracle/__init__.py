@@ -12,6 +12,7 @@ from .oracle import (  # noqa: F401
     activation,
     build,
     max_threads,
+    pack_weights,
     silu,
     swiglu_oracle,
     swiglu_oracle_rows,

@@ -54,6 +54,8 @@ def _load():
         lib.swiglu_oracle_activation.restype = ctypes.c_double
         lib.swiglu_oracle_silu.argtypes = [ctypes.c_double]
         lib.swiglu_oracle_silu.restype = ctypes.c_double
+        lib.swiglu_oracle_pack.argtypes = [p, p, p, i64, i64]
+        lib.swiglu_oracle_pack.restype = ctypes.c_int
         lib.swiglu_oracle_max_threads.argtypes = []
         lib.swiglu_oracle_max_threads.restype = ctypes.c_int
         _lib = lib
@@ -133,3 +135,16 @@ def swiglu_oracle_rows(A_bits, W1_bits, W2_bits, rows, nthreads: int = 0, act=0)
     if used < 0:
         raise RuntimeError("swiglu_oracle_rows rejected its arguments")
     return Y, int(used)
+
+
+def pack_weights(W1_bits, W2_bits):
+    """The one-time W_fused interleave (swiglu_oracle.c
+    swiglu_oracle_pack): uint16 [ceil(N/128), 4, K, 64] from W1, W2 [K, N] bit patterns."""
+    W1_bits = np.ascontiguousarray(W1_bits)
+    K, N = W1_bits.shape
+    W1 = _bits(W1_bits, (K, N), "W1")
+    W2 = _bits(W2_bits, (K, N), "W2")
+    Wp = np.empty(((N + 127) // 128, 4, K, 64), dtype=np.uint16)
+    if _load().swiglu_oracle_pack(_ptr(W1), _ptr(W2), _ptr(Wp), N, K) != 0:
+        raise RuntimeError("swiglu_oracle_pack rejected its arguments")
+    return Wp

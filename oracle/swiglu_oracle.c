@@ -200,6 +200,36 @@ int swiglu_oracle_rows(const uint16_t *A, const uint16_t *W1, const uint16_t *W2
   return swiglu_oracle_rows_act(A, W1, W2, Ysub, rows, count, M, N, K, 0, nthreads);
 }
 
+/*
+ * The one-time weight interleave ("W_fused"): Kernel-2
+ * "interleaves W1 and W2" ahead of time so that a Gate column and its Up column reach the same
+ * tile.  The paper does not print the layout; the reading taken (R18) interleaves
+ * 64-column slabs inside 128-column tiles:
+ *
+ *     Wp[t][s][k][c],  t < ceil(N/128), s in {0,1,2,3} = {gate 0, up 0, gate 1, up 1}, c < 64
+ *       = W1[k][128 t + 64 (s/2) + c]   if s is even
+ *       = W2[k][128 t + 64 (s/2) + c]   if s is odd
+ *       = 0                             where that column is >= N
+ *
+ * Pure index work on 16-bit patterns, written as the definition: one loop per index.
+ * Pins (tests/test_oracle_pack_pins.py): every (k, n) of W1 and of W2 appears exactly once, at
+ * the stated position (checked by an independent inverse walk), padding is zero, a tiny case
+ * written out by hand in tests/golden/.
+ */
+int swiglu_oracle_pack(const uint16_t* W1, const uint16_t* W2, uint16_t* Wp, int64_t N, int64_t K) {
+  if (!W1 || !W2 || !Wp || N <= 0 || K <= 0) return -1;
+  const int64_t tiles = (N + 127) / 128;
+  for (int64_t t = 0; t < tiles; ++t)
+    for (int64_t s = 0; s < 4; ++s)
+      for (int64_t k = 0; k < K; ++k)
+        for (int64_t c = 0; c < 64; ++c) {
+          const int64_t n = 128 * t + 64 * (s / 2) + c;
+          const uint16_t* W = (s % 2 == 0) ? W1 : W2;
+          Wp[((t * 4 + s) * K + k) * 64 + c] = (n < N) ? W[k * N + n] : (uint16_t)0;
+        }
+  return 0;
+}
+
 int swiglu_oracle_max_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

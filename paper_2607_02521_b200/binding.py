@@ -32,7 +32,8 @@ EXPORTS = (
     "swiglu_selected_variant", "swiglu_launches_per_call", "swiglu_validate",
     "swiglu_mlp_host", "swiglu_last_error", "swiglu_status_string", "swiglu_version",
     "swiglu_release", "swiglu_release_stream", "swiglu_reload_env", "swiglu_tensor_map_cache_stats",
-    "swiglu_set_clock_probe",
+    "swiglu_set_clock_probe", "swiglu_packed_weight_bytes", "swiglu_pack_weights",
+    "swiglu_mlp_packed", "swiglu_glu_mlp_packed", "swiglu_launch_floor_probe",
 )
 
 
@@ -87,6 +88,13 @@ def load():
     u64p = ctypes.POINTER(ctypes.c_uint64)
     lib.swiglu_tensor_map_cache_stats.argtypes, lib.swiglu_tensor_map_cache_stats.restype = [u64p, u64p], ci
     lib.swiglu_set_clock_probe.argtypes, lib.swiglu_set_clock_probe.restype = [p], None
+    lib.swiglu_packed_weight_bytes.argtypes, lib.swiglu_packed_weight_bytes.restype = [i64, i64], sz
+    lib.swiglu_pack_weights.argtypes, lib.swiglu_pack_weights.restype = [p, p, p, i64, i64, ci, p], ci
+    lib.swiglu_mlp_packed.argtypes, lib.swiglu_mlp_packed.restype = [p, p, p, i64, i64, i64, p], ci
+    lib.swiglu_glu_mlp_packed.argtypes = [p, p, p, i64, i64, i64, ci, ci, p]
+    lib.swiglu_glu_mlp_packed.restype = ci
+    lib.swiglu_launch_floor_probe.argtypes = [p, p, p, p, i64, i64, i64, p]
+    lib.swiglu_launch_floor_probe.restype = ci
     lib.swiglu_last_error.argtypes, lib.swiglu_last_error.restype = [], ctypes.c_char_p
     lib.swiglu_status_string.argtypes, lib.swiglu_status_string.restype = [ci], ctypes.c_char_p
     lib.swiglu_version.argtypes, lib.swiglu_version.restype = [], ctypes.c_char_p
@@ -298,6 +306,41 @@ def swiglu_tensor_map_cache_stats():
     h, m = ctypes.c_uint64(0), ctypes.c_uint64(0)
     slots = load().swiglu_tensor_map_cache_stats(ctypes.byref(h), ctypes.byref(m))
     return int(h.value), int(m.value), int(slots)
+
+
+def swiglu_packed_weight_bytes(N, K) -> int:
+    return int(load().swiglu_packed_weight_bytes(int(N), int(K)))
+
+
+def swiglu_pack_weights(W1, W2, Wp, N, K, weight_layout=WEIGHTS_KN, stream=None) -> None:
+    """One-time prepack of (W1, W2) into the tile-interleaved W_fused buffer Wp (device)."""
+    _check(load().swiglu_pack_weights(_ptr(W1), _ptr(W2), _ptr(Wp), int(N), int(K),
+                                      int(weight_layout), _stream(stream)))
+
+
+def swiglu_mlp_packed(A, Wp, Y, M=None, N=None, K=None, stream=None) -> None:
+    """Fused Y = bf16(SiLU(A.W1) * (A.W2)) from prepacked weights (see the header's contract)."""
+    if M is None:
+        M, K = int(A.shape[0]), int(A.shape[1])
+        N = int(Y.shape[1])
+    _check(load().swiglu_mlp_packed(_ptr(A), _ptr(Wp), _ptr(Y), int(M), int(N), int(K),
+                                    _stream(stream)))
+
+
+def swiglu_glu_mlp_packed(A, Wp, Y, activation="silu", variant=-1, M=None, N=None, K=None,
+                          stream=None) -> None:
+    if M is None:
+        M, K = int(A.shape[0]), int(A.shape[1])
+        N = int(Y.shape[1])
+    _check(load().swiglu_glu_mlp_packed(_ptr(A), _ptr(Wp), _ptr(Y), int(M), int(N), int(K),
+                                        _act(activation), int(variant), _stream(stream)))
+
+
+def swiglu_launch_floor_probe(A, W1, W2, Y, M=None, N=None, K=None, stream=None) -> None:
+    """Measurement aid: the decode kernel's launch with an empty body (see the header)."""
+    m, n, k = _dims(A, W1, W2, Y, M, N, K)
+    _check(load().swiglu_launch_floor_probe(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), m, n, k,
+                                            _stream(stream)))
 
 
 def swiglu_set_clock_probe(buf) -> None:

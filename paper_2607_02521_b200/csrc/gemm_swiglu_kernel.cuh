@@ -158,18 +158,30 @@ __device__ __forceinline__ float glu_mul(float g, float u) {
   }
 }
 
-// kWK = false: weights are [K,N] row-major (N contiguous; the paper's layout, PAPER.md lines
-//   94, 206) -- an MN-major UMMA "B" operand.  kWK = true: weights are [N,K] row-major (K
-//   contiguous, the nn.Linear layout serving stacks store, lines 72-74) -- a K-major operand.
+// Weight source (kWMode):
+//   kWeightsKN: [K,N] row-major (N contiguous; the paper's layout) -- an
+//     MN-major UMMA "B" operand.
+//   kWeightsNK: [N,K] row-major (K contiguous, the nn.Linear layout serving stacks store, lines
+//     72-74) -- a K-major operand.
 //   Either way a 64-column slab of a weight tile is one 8 KB TMA box (64 x 64 bf16, 128-byte
-//   swizzle) and the slabs W1[0:64) W1[64:128) W2[0:64) W2[64:128) sit 8 KB apart.
-template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = kActSilu, bool kWK = false>
+//   swizzle) and the slabs W1[0:64) W1[64:128) W2[0:64) W2[64:128) sit 8 KB apart in smem.
+//   kWeightsPacked: the tile-interleaved W_fused of swiglu_pack_weights (the sm_100 form of the
+//     paper's Kernel-2 one-time interleave, lines 159, 167-169): slab-major
+//     [n-tile][g0,u0,g1,u1][K][64], so ONE 3-D TMA box per stage fetches Gate|Up slabs
+//     (tmap_b1: the multi-slab box; tmap_b2: a single-slab box for 2-CTA / 1-CTA half tiles).
+//     MN-major like KN; accumulator columns come out as g0 u0 g1 u1.
+enum : int { kWeightsKN = 0, kWeightsNK = 1, kWeightsPacked = 2 };
+
+template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = kActSilu, int kWMode = kWeightsKN>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                    const __grid_constant__ CUtensorMap tmap_b1,
                    const __grid_constant__ CUtensorMap tmap_b2,
                    const __grid_constant__ CUtensorMap tmap_y, const GemmParams p) {
   static_assert(kBN == 128 || (kBN == 64 && kFused && kCtaGroup == 1), "narrow tile: fused 1-CTA");
+  static_assert(kWMode != kWeightsPacked || kFused, "packed weights: fused path only");
+  constexpr bool kWK = (kWMode == kWeightsNK);
+  constexpr bool kPacked = (kWMode == kWeightsPacked);
   constexpr int UMMA_N = kFused ? 2 * kBN : 256;  // accumulator columns per tile
   using Cfg = GemmCfg<kCtaGroup, UMMA_N>;
   constexpr int kStages = Cfg::kStages;
@@ -214,7 +226,23 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       if constexpr (kCtaGroup == 1) tma_load_2d(dst, tm, fb, kWK ? k0 : n, kWK ? n : k0, w_policy);
       else tma_load_2d_pair(dst, tm, fb, kWK ? k0 : n, kWK ? n : k0, w_policy);
     };
-    if constexpr (kCtaGroup == 1) {
+    if constexpr (kPacked) {
+      // slab index of (n_base, Gate): tiles of 128 columns hold 4 slabs g0 u0 g1 u1
+      const int slab = (n_base >> 7) * 4 + ((n_base >> 6) & 1) * 2;
+      if constexpr (kCtaGroup == 1) {
+        tma_load_2d(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
+        if (half) {  // g_h | u_h as two single-slab boxes
+          tma_load_3d(sb, &tmap_b2, fb, 0, k0, slab, w_policy);
+          tma_load_3d(sb + 8192, &tmap_b2, fb, 0, k0, slab + 1, w_policy);
+        } else {     // one box: 4 slabs (128-column tile) or 2 slabs (64-column tile)
+          tma_load_3d(sb, &tmap_b1, fb, 0, k0, slab, w_policy);
+        }
+      } else {
+        tma_load_2d_pair(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
+        if (half) tma_load_3d_pair(sb, &tmap_b2, fb, 0, k0, slab + (int)rank, w_policy);
+        else tma_load_3d_pair(sb, &tmap_b1, fb, 0, k0, slab + 2 * (int)rank, w_policy);
+      }
+    } else if constexpr (kCtaGroup == 1) {
       tma_load_2d(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
       if constexpr (kFused) {
         if (kBN == 64 || half) {  // W1 slab | W2 slab
@@ -377,8 +405,11 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           uint32_t packed[16];
           if constexpr (kFused) {
             uint32_t g[32], u[32];
-            tmem_ld_32x32b_x32(tacc + h * 64 + c * 32, g);
-            tmem_ld_32x32b_x32(tacc + w + h * 64 + c * 32, u);  // Up starts at column w
+            // accumulator columns: [Gate w | Up w], or g0 u0 g1 u1 for packed weights
+            const uint32_t gcol = kPacked ? h * 128 + c * 32 : h * 64 + c * 32;
+            const uint32_t ucol = kPacked ? gcol + 64 : gcol + w;
+            tmem_ld_32x32b_x32(tacc + gcol, g);
+            tmem_ld_32x32b_x32(tacc + ucol, u);
             tmem_ld_wait();
 #pragma unroll
             for (int j = 0; j < 16; ++j) {

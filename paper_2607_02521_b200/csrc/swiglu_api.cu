@@ -18,6 +18,10 @@
 
 namespace {
 
+using swiglu::kWeightsKN;
+using swiglu::kWeightsNK;
+using swiglu::kWeightsPacked;
+
 // ------------------------------------------------------------------ error bookkeeping
 thread_local char g_err[512] = "";
 
@@ -192,7 +196,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 EncodeTiledFn g_encode = nullptr;
 
 // Opt every fused kernel of activation kAct in to its dynamic shared-memory size.
-template <int kAct, bool kWK>
+template <int kAct, int kWK>
 int set_smem_attrs() {
   using namespace swiglu;
   const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
@@ -203,7 +207,7 @@ int set_smem_attrs() {
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kAct, kWK>, attr, SmallCfg<32>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kAct, kWK>, attr, SmallCfg<64>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<128, kAct, kWK>, attr, SmallCfg<128>::kSmemBytes));
-  if (kAct == kActSilu) {  // the unfused path's plain GEMMs have no activation
+  if constexpr (kAct == kActSilu && kWK != kWeightsPacked) {  // the unfused path's plain GEMMs have no activation
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kActSilu, kWK, true>, attr, SmallCfg<16>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kActSilu, kWK, true>, attr, SmallCfg<32>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kActSilu, kWK, true>, attr, SmallCfg<64>::kSmemBytes));
@@ -239,10 +243,12 @@ int get_device_state(DeviceState** out) {
     }
     using namespace swiglu;
     int rc;
-    if ((rc = set_smem_attrs<kActSilu, false>()) || (rc = set_smem_attrs<kActGelu, false>()) ||
-        (rc = set_smem_attrs<kActGeluTanh, false>()) || (rc = set_smem_attrs<kActRelu, false>()) ||
-        (rc = set_smem_attrs<kActSilu, true>()) || (rc = set_smem_attrs<kActGelu, true>()) ||
-        (rc = set_smem_attrs<kActGeluTanh, true>()) || (rc = set_smem_attrs<kActRelu, true>()))
+    if ((rc = set_smem_attrs<kActSilu, kWeightsKN>()) || (rc = set_smem_attrs<kActGelu, kWeightsKN>()) ||
+        (rc = set_smem_attrs<kActGeluTanh, kWeightsKN>()) || (rc = set_smem_attrs<kActRelu, kWeightsKN>()) ||
+        (rc = set_smem_attrs<kActSilu, kWeightsNK>()) || (rc = set_smem_attrs<kActGelu, kWeightsNK>()) ||
+        (rc = set_smem_attrs<kActGeluTanh, kWeightsNK>()) || (rc = set_smem_attrs<kActRelu, kWeightsNK>()) ||
+        (rc = set_smem_attrs<kActSilu, kWeightsPacked>()) || (rc = set_smem_attrs<kActGelu, kWeightsPacked>()) ||
+        (rc = set_smem_attrs<kActGeluTanh, kWeightsPacked>()) || (rc = set_smem_attrs<kActRelu, kWeightsPacked>()))
       return rc;
     d.ready = true;
   }
@@ -251,13 +257,13 @@ int get_device_state(DeviceState** out) {
 }
 
 // Tensor-map cache (a0: "build or fetch cached CUtensorMaps").  A map is a pure function of
-// (base, inner, outer, box): a cached copy can never be stale, whatever happened to the
+// (base, dims, box): a cached copy can never be stale, whatever happened to the
 // allocation in between.  Thread-local and direct-mapped, so the hot path takes no lock.
 struct TmapKey {
-  const void* base; int64_t inner, outer; uint32_t box_inner, box_outer;
+  const void* base; int64_t d0, d1, d2; uint32_t b0, b1, b2;
   bool operator==(const TmapKey& o) const {
-    return base == o.base && inner == o.inner && outer == o.outer && box_inner == o.box_inner &&
-           box_outer == o.box_outer;
+    return base == o.base && d0 == o.d0 && d1 == o.d1 && d2 == o.d2 && b0 == o.b0 && b1 == o.b1 &&
+           b2 == o.b2;
   }
 };
 struct TmapSlot { bool used = false; TmapKey key; CUtensorMap map; };
@@ -265,18 +271,29 @@ constexpr int kTmapSlots = 256;
 thread_local TmapSlot t_tmaps[kTmapSlots];
 thread_local uint64_t t_tmap_hits = 0, t_tmap_misses = 0;
 
-int encode_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
-                uint32_t box_inner, uint32_t box_outer);
+// bf16 tensor, dense row-major, dims innermost first (d2 == 0: 2-D), box b0 x b1 [x b2],
+// 128-byte swizzle (b0 must be 64 elements), out-of-bounds reads give zeros.
+int encode_tmap(CUtensorMap* out, const TmapKey& k) {
+  const cuuint32_t rank = k.d2 ? 3 : 2;
+  const cuuint64_t dims[3] = {(cuuint64_t)k.d0, (cuuint64_t)k.d1, (cuuint64_t)k.d2};
+  const cuuint64_t strides[2] = {(cuuint64_t)k.d0 * 2, (cuuint64_t)k.d0 * 2 * (cuuint64_t)k.d1};
+  const cuuint32_t box[3] = {k.b0, k.b1, k.b2};
+  const cuuint32_t elem[3] = {1, 1, 1};
+  const CUresult r =
+      g_encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, rank, const_cast<void*>(k.base), dims,
+               strides, box, elem, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS)
+    return fail(SWIGLU_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d) dims=%lld x %lld x %lld",
+                (int)r, (long long)k.d0, (long long)k.d1, (long long)k.d2);
+  return SWIGLU_OK;
+}
 
-// 2-D bf16 row-major tensor [outer, inner] (inner contiguous), box = box_outer x box_inner,
-// 128-byte swizzle (box_inner must be 64 elements), out-of-bounds reads give zeros.
-int make_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
-              uint32_t box_inner, uint32_t box_outer) {
-  if (env().no_tmap_cache) return encode_tmap(out, base, inner, outer, box_inner, box_outer);
-  const TmapKey key{base, inner, outer, box_inner, box_outer};
-  uint64_t h = (uint64_t)(uintptr_t)base * 0x9E3779B97F4A7C15ull;
-  h ^= ((uint64_t)inner * 0xC2B2AE3D27D4EB4Full) ^ ((uint64_t)outer * 0x165667B19E3779F9ull) ^
-       ((uint64_t)box_outer << 7) ^ box_inner;
+int cached_tmap(CUtensorMap* out, const TmapKey& key) {
+  if (env().no_tmap_cache) return encode_tmap(out, key);
+  uint64_t h = (uint64_t)(uintptr_t)key.base * 0x9E3779B97F4A7C15ull;
+  h ^= ((uint64_t)key.d0 * 0xC2B2AE3D27D4EB4Full) ^ ((uint64_t)key.d1 * 0x165667B19E3779F9ull) ^
+       ((uint64_t)key.d2 * 0x27D4EB2F165667C5ull) ^ ((uint64_t)key.b1 << 7) ^ ((uint64_t)key.b2 << 17);
   TmapSlot& slot = t_tmaps[(h >> 40) & (kTmapSlots - 1)];
   if (slot.used && slot.key == key) {
     ++t_tmap_hits;
@@ -284,7 +301,7 @@ int make_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
     return SWIGLU_OK;
   }
   ++t_tmap_misses;
-  const int rc = encode_tmap(out, base, inner, outer, box_inner, box_outer);
+  const int rc = encode_tmap(out, key);
   if (rc) return rc;
   slot.used = true;
   slot.key = key;
@@ -292,35 +309,40 @@ int make_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
   return SWIGLU_OK;
 }
 
-int encode_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
-                uint32_t box_inner, uint32_t box_outer) {
-  const cuuint64_t dims[2] = {(cuuint64_t)inner, (cuuint64_t)outer};
-  const cuuint64_t strides[1] = {(cuuint64_t)inner * 2};
-  const cuuint32_t box[2] = {box_inner, box_outer};
-  const cuuint32_t elem[2] = {1, 1};
-  const CUresult r =
-      g_encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides,
-               box, elem, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS)
-    return fail(SWIGLU_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d) inner=%lld outer=%lld",
-                (int)r, (long long)inner, (long long)outer);
-  return SWIGLU_OK;
+// 2-D tensor [outer, inner] (inner contiguous), box = box_outer x box_inner.
+int make_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
+              uint32_t box_inner, uint32_t box_outer) {
+  return cached_tmap(out, TmapKey{base, inner, outer, 0, box_inner, box_outer, 0});
 }
+// Prepacked weights Wp[slab][k][64]: {64, K, slabs}, box = 64 x 64 x box_slabs.
+int make_tmap_packed(CUtensorMap* out, const void* base, int64_t K, int64_t slabs,
+                     uint32_t box_slabs) {
+  return cached_tmap(out, TmapKey{base, 64, K, slabs, 64, 64, box_slabs});
+}
+inline int64_t packed_slabs(int64_t N) { return 4 * ((N + 127) / 128); }
 
 bool pdl_enabled() { return !env().no_pdl; }
 
 // ------------------------------------------------------------------ launches
-template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = swiglu::kActSilu, bool kWK = false>
+template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = swiglu::kActSilu, int kWMode = 0>
 int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void* B2, void* Yout,
                 int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
   using namespace swiglu;
   CUtensorMap ta, tb1, tb2, ty;
   int rc;
+  constexpr bool kWK = (kWMode == kWeightsNK);
   if ((rc = make_tmap(&ta, A, K, M, 64, 128))) return rc;
-  // weights: [K,N] (inner N) or [N,K] (inner K); a box is always one 64 x 64 slab
-  if ((rc = make_tmap(&tb1, B1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
-  if ((rc = make_tmap(&tb2, kFused ? B2 : B1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
+  if constexpr (kWMode == kWeightsPacked) {
+    // B1 = Wp: one box per stage -- 4 slabs (1-CTA, 128 columns) or 2 (64-column tile; each
+    // CTA of a pair); single-slab boxes for the half tiles of the last wave
+    const uint32_t box = (kCtaGroup == 1 && kBN == 128) ? 4 : 2;
+    if ((rc = make_tmap_packed(&tb1, B1, K, packed_slabs(N), box))) return rc;
+    if ((rc = make_tmap_packed(&tb2, B1, K, packed_slabs(N), 1))) return rc;
+  } else {
+    // weights: [K,N] (inner N) or [N,K] (inner K); a box is always one 64 x 64 slab
+    if ((rc = make_tmap(&tb1, B1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
+    if ((rc = make_tmap(&tb2, kFused ? B2 : B1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
+  }
   if ((rc = make_tmap(&ty, Yout, N, M, 64, 128))) return rc;
   using Cfg = GemmCfg<kCtaGroup, kFused ? 2 * kBN : 256>;
   GemmParams p;
@@ -380,8 +402,8 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   }
   cfg.attrs = attrs;
   cfg.numAttrs = na;
-  CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_swiglu_kernel<kCtaGroup, kFused, kBN, kAct, kWK>, ta, tb1,
-                              tb2, ty, p));
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_swiglu_kernel<kCtaGroup, kFused, kBN, kAct, kWMode>, ta,
+                              tb1, tb2, ty, p));
   return SWIGLU_OK;
 }
 
@@ -410,21 +432,29 @@ int smallm_ksplit(int sm_count, int ctas_per_sm, int mp, int64_t n_tiles, int64_
   return (int)s;
 }
 
-template <int MP, int kAct, bool kWK, bool kStoreGU = false>
+template <int MP, int kAct, int kWMode, bool kStoreGU = false>
 int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const void* W2,
-                     void* Y, void* U, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
+                     void* Y, void* U, int64_t M, int64_t N, int64_t K, cudaStream_t stream,
+                     int probe = 0) {
   using namespace swiglu;
+  constexpr bool kWK = (kWMode == kWeightsNK);
   CUtensorMap ta, tw1, tw2;
   int rc;
   if ((rc = make_tmap(&ta, A, K, M, 64, MP))) return rc;
-  if ((rc = make_tmap(&tw1, W1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
-  if ((rc = make_tmap(&tw2, W2, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
+  if constexpr (kWMode == kWeightsPacked) {
+    if ((rc = make_tmap_packed(&tw1, W1, K, packed_slabs(N), 4))) return rc;  // W1 = Wp
+    tw2 = tw1;
+  } else {
+    if ((rc = make_tmap(&tw1, W1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
+    if ((rc = make_tmap(&tw2, W2, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
+  }
   const int64_t n_tiles = (N + 127) / 128, k_blocks = (K + BK - 1) / BK;
   SmallParams p;
   p.M = (int)M; p.N = (int)N; p.K = (int)K;
   p.ksplit = smallm_ksplit(d.sm_count, SmallCfg<MP>::kCtasPerSm, MP, n_tiles, k_blocks);
   p.ldy = N;
   p.U = (uint16_t*)U;
+  p.probe = probe;
   p.clk = g_clk.load(std::memory_order_relaxed);
   // L2 prefetch ahead of the grid dependency: at most ~32 MiB over the whole grid
   const int64_t grid = n_tiles * p.ksplit;
@@ -457,18 +487,18 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   }
   cfg.attrs = attrs;
   cfg.numAttrs = na;
-  CUDA_TRY(cudaLaunchKernelEx(&cfg, smallm_swiglu_kernel<MP, kAct, kWK, kStoreGU>, ta, tw1, tw2,
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, smallm_swiglu_kernel<MP, kAct, kWMode, kStoreGU>, ta, tw1, tw2,
                               (uint16_t*)Y, p));
   return SWIGLU_OK;
 }
 
-template <int kAct, bool kWK, bool kStoreGU = false>
+template <int kAct, int kWMode, bool kStoreGU = false>
 int launch_smallm(const DeviceState& d, const void* A, const void* W1, const void* W2, void* Y,
-                  void* U, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
-  if (M <= 16) return launch_smallm_mp<16, kAct, kWK, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream);
-  if (M <= 32) return launch_smallm_mp<32, kAct, kWK, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream);
-  if (M <= 64) return launch_smallm_mp<64, kAct, kWK, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream);
-  return launch_smallm_mp<128, kAct, kWK, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream);
+                  void* U, int64_t M, int64_t N, int64_t K, cudaStream_t stream, int probe = 0) {
+  if (M <= 16) return launch_smallm_mp<16, kAct, kWMode, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream, probe);
+  if (M <= 32) return launch_smallm_mp<32, kAct, kWMode, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream, probe);
+  if (M <= 64) return launch_smallm_mp<64, kAct, kWMode, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream, probe);
+  return launch_smallm_mp<128, kAct, kWMode, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream, probe);
 }
 
 template <int kAct>
@@ -563,7 +593,7 @@ int release_pool(std::map<cudaStream_t, DeviceState::Buf>& pool, bool all, cudaS
   return SWIGLU_OK;
 }
 
-template <int kAct, bool kWK>
+template <int kAct, int kWK>
 int launch_fused_l(const DeviceState& d, int variant, const void* A, const void* W1,
                    const void* W2, void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
   switch (variant) {
@@ -577,16 +607,25 @@ int launch_fused_l(const DeviceState& d, int variant, const void* A, const void*
 template <int kAct>
 int launch_fused(const DeviceState& d, int variant, int layout, const void* A, const void* W1,
                  const void* W2, void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
-  return layout ? launch_fused_l<kAct, true>(d, variant, A, W1, W2, Y, M, N, K, stream)
-                : launch_fused_l<kAct, false>(d, variant, A, W1, W2, Y, M, N, K, stream);
+  switch (layout) {
+    case kWeightsNK: return launch_fused_l<kAct, kWeightsNK>(d, variant, A, W1, W2, Y, M, N, K, stream);
+    case kWeightsPacked: return launch_fused_l<kAct, kWeightsPacked>(d, variant, A, W1, W2, Y, M, N, K, stream);
+  }
+  return launch_fused_l<kAct, kWeightsKN>(d, variant, A, W1, W2, Y, M, N, K, stream);
 }
 
+// layout: SWIGLU_WEIGHTS_KN / _NK, or kWeightsPacked (internal: W1 = W2 = the packed buffer).
 int run_fused(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
               int64_t K, int variant, int act, int layout, cudaStream_t stream) {
-  if (layout != SWIGLU_WEIGHTS_KN && layout != SWIGLU_WEIGHTS_NK)
+  if (layout != SWIGLU_WEIGHTS_KN && layout != SWIGLU_WEIGHTS_NK && layout != kWeightsPacked)
     return fail(SWIGLU_ERR_UNSUPPORTED, "unknown weight layout %d", layout);
   int rc = validate(A, W1, W2, Y, M, N, K);
   if (rc) return rc;
+  if (layout == kWeightsPacked && M > 0) {
+    // the packed buffer is 2 * K * pad128(N) elements: re-check aliasing against its real size
+    const int64_t pb = 2 * K * ((N + 127) / 128 * 128) * 2;
+    if (overlaps(Y, M * N * 2, W1, pb)) return fail(SWIGLU_ERR_ALIASING, "Y overlaps Wp");
+  }
   if (act < 0 || act >= swiglu::kNumActs)
     return fail(SWIGLU_ERR_UNSUPPORTED, "unknown activation %d", act);
   if (variant < -1 || variant >= kNumFused)
@@ -634,23 +673,23 @@ int run_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t 
   if (variant < 0) variant = select_unfused(M, N, K);
   void* G = ws;
   void* U = (char*)ws + need / 2;
-  using swiglu::kActSilu;
+  using namespace swiglu;
   if (variant == kUnfusedSmallM) {
-    rc = layout ? launch_smallm<kActSilu, true, true>(*d, A, W1, W2, G, U, M, N, K, stream)
-                : launch_smallm<kActSilu, false, true>(*d, A, W1, W2, G, U, M, N, K, stream);
+    rc = layout ? launch_smallm<kActSilu, kWeightsNK, true>(*d, A, W1, W2, G, U, M, N, K, stream)
+                : launch_smallm<kActSilu, kWeightsKN, true>(*d, A, W1, W2, G, U, M, N, K, stream);
     if (rc) return rc;
   } else if (variant == kUnfused1Cta && !layout) {
     if ((rc = launch_gemm<1, false>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
     if ((rc = launch_gemm<1, false>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
   } else if (variant == kUnfused1Cta) {
-    if ((rc = launch_gemm<1, false, 128, kActSilu, true>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
-    if ((rc = launch_gemm<1, false, 128, kActSilu, true>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
+    if ((rc = launch_gemm<1, false, 128, kActSilu, kWeightsNK>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
+    if ((rc = launch_gemm<1, false, 128, kActSilu, kWeightsNK>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
   } else if (!layout) {
     if ((rc = launch_gemm<2, false>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
     if ((rc = launch_gemm<2, false>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
   } else {
-    if ((rc = launch_gemm<2, false, 128, kActSilu, true>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
-    if ((rc = launch_gemm<2, false, 128, kActSilu, true>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
+    if ((rc = launch_gemm<2, false, 128, kActSilu, kWeightsNK>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
+    if ((rc = launch_gemm<2, false, 128, kActSilu, kWeightsNK>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
   }
   return launch_silu_mul(*d, G, U, Y, M * N, act, stream);
 }
@@ -704,6 +743,8 @@ int swiglu_glu_mlp_unfused(const void* A, const void* W1, const void* W2, void* 
 int swiglu_glu_mlp_layout(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
                           int64_t N, int64_t K, int activation, int weight_layout, int unfused,
                           int variant, void* stream) {
+  if (weight_layout != SWIGLU_WEIGHTS_KN && weight_layout != SWIGLU_WEIGHTS_NK)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "unknown weight layout %d", weight_layout);
   if (unfused)
     return run_unfused(A, W1, W2, Y, M, N, K, nullptr, 0, true, variant, activation,
                        weight_layout, (cudaStream_t)stream);
@@ -714,6 +755,64 @@ int swiglu_glu_mlp_layout(const void* A, const void* W1, const void* W2, void* Y
 int swiglu_glu_mlp_ex(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
                       int64_t N, int64_t K, int activation, int variant, void* stream) {
   return run_fused(A, W1, W2, Y, M, N, K, variant, activation, 0, (cudaStream_t)stream);
+}
+
+size_t swiglu_packed_weight_bytes(int64_t N, int64_t K) {
+  if (N <= 0 || K <= 0 || (N % 8) || (K % 8)) return 0;
+  return (size_t)2 * (size_t)K * (size_t)((N + 127) / 128 * 128) * 2;
+}
+
+int swiglu_pack_weights(const void* W1, const void* W2, void* Wp, int64_t N, int64_t K,
+                        int weight_layout, void* stream) {
+  if (weight_layout != SWIGLU_WEIGHTS_KN && weight_layout != SWIGLU_WEIGHTS_NK)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "unknown weight layout %d", weight_layout);
+  // same shape / pointer rules as a compute call with one row (Wp plays the part of Y)
+  int rc = validate(W1, W1, W2, Wp, 1, N, K);
+  if (rc == SWIGLU_ERR_ALIASING) rc = SWIGLU_OK;  // checked against the real sizes below
+  if (rc) return rc;
+  const int64_t wb = K * N * 2, pb = (int64_t)swiglu_packed_weight_bytes(N, K);
+  if (overlaps(Wp, pb, W1, wb) || overlaps(Wp, pb, W2, wb))
+    return fail(SWIGLU_ERR_ALIASING, "Wp overlaps W1 or W2");
+  DeviceState* d;
+  if ((rc = get_device_state(&d))) return rc;
+  const long long total_vec = pb / 16;
+  long long blocks = (total_vec + 255) / 256;
+  const long long cap = (long long)d->sm_count * 16;
+  if (blocks > cap) blocks = cap;
+  if (weight_layout == SWIGLU_WEIGHTS_NK)
+    swiglu::pack_weights_kernel<true><<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(
+        (const uint16_t*)W1, (const uint16_t*)W2, (uint16_t*)Wp, (int)N, (int)K, total_vec);
+  else
+    swiglu::pack_weights_kernel<false><<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(
+        (const uint16_t*)W1, (const uint16_t*)W2, (uint16_t*)Wp, (int)N, (int)K, total_vec);
+  CUDA_TRY(cudaGetLastError());
+  return SWIGLU_OK;
+}
+
+int swiglu_mlp_packed(const void* A, const void* Wp, void* Y, int64_t M, int64_t N, int64_t K,
+                      void* stream) {
+  return run_fused(A, Wp, Wp, Y, M, N, K, -1, swiglu::kActSilu, swiglu::kWeightsPacked,
+                   (cudaStream_t)stream);
+}
+
+int swiglu_glu_mlp_packed(const void* A, const void* Wp, void* Y, int64_t M, int64_t N, int64_t K,
+                          int activation, int variant, void* stream) {
+  return run_fused(A, Wp, Wp, Y, M, N, K, variant, activation, swiglu::kWeightsPacked,
+                   (cudaStream_t)stream);
+}
+
+int swiglu_launch_floor_probe(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                              int64_t N, int64_t K, void* stream) {
+  int rc = validate(A, W1, W2, Y, M, N, K);
+  if (rc) return rc;
+  if (M == 0) return SWIGLU_OK;
+  if (M > swiglu::kSmallMMax)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "the launch-floor probe mirrors the small-M kernel: M <= %d",
+                swiglu::kSmallMMax);
+  DeviceState* d;
+  if ((rc = get_device_state(&d))) return rc;
+  return launch_smallm<swiglu::kActSilu, swiglu::kWeightsKN>(*d, A, W1, W2, Y, nullptr, M, N, K,
+                                                             (cudaStream_t)stream, /*probe=*/1);
 }
 
 const char* swiglu_activation_name(int activation) {

@@ -1,0 +1,176 @@
+"""Prepacked tile-interleaved weights:
+the pack kernel bit-exact against the oracle's interleave, and swiglu_mlp_packed against the
+fp64 oracle of Eq. 1-3 on the ORIGINAL W1, W2 -- every fused variant, ragged M / N / K, both
+input layouts, every activation, CUDA-graph chains (where the decode kernel loads the packed
+weights ahead of griddepcontrol.wait)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2607_02521_b200 import binding as B
+from paper_2607_02521_b200 import check, inputs
+
+pytestmark = pytest.mark.gpu
+ATOL, RTOL = 2e-3, 1.6e-2
+
+
+def dev(bits):
+    return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).cuda().view(torch.bfloat16)
+
+
+def host(t):
+    return t.view(torch.int16).cpu().numpy().view(np.uint16)
+
+
+def pack(W1, W2, layout=B.WEIGHTS_KN):
+    K, N = W1.shape
+    nbytes = B.swiglu_packed_weight_bytes(N, K)
+    assert nbytes == 2 * K * ((N + 127) // 128 * 128) * 2
+    buf = torch.full((nbytes // 2 + 64,), -21846, dtype=torch.int16, device="cuda")  # + guard
+    Wp = buf[:nbytes // 2]
+    if layout == B.WEIGHTS_KN:
+        B.swiglu_pack_weights(dev(W1), dev(W2), Wp, N, K, layout)
+    else:
+        B.swiglu_pack_weights(dev(np.ascontiguousarray(W1.T)), dev(np.ascontiguousarray(W2.T)), Wp, N, K, layout)
+    torch.cuda.synchronize()
+    assert bool((buf[nbytes // 2:] == -21846).all()), "pack wrote past the packed buffer"
+    return Wp
+
+
+def assert_parity(y_bits, y_ref, what):
+    rep = check.compare(y_bits, y_ref)
+    y = inputs.bf16_bits_to_f64(y_bits)
+    assert np.all(np.isfinite(y)), what
+    assert np.all(np.abs(y - y_ref) <= ATOL + RTOL * np.abs(y_ref)), (what, rep)
+    return rep
+
+
+@pytest.mark.parametrize("layout", [B.WEIGHTS_KN, B.WEIGHTS_NK])
+@pytest.mark.parametrize("K,N", [(8, 8), (72, 136), (200, 264), (64, 128), (896, 4864), (328, 1160)])
+def test_pack_kernel_is_bit_exact(K, N, layout):
+    _, W1, W2 = inputs.make_case(1, N, K, seed=1000 + N + K)
+    Wp = pack(W1, W2, layout)
+    want = oracle.pack_weights(W1, W2)
+    got = Wp.cpu().numpy().view(np.uint16).reshape(want.shape)
+    assert np.array_equal(got, want)
+
+
+SHAPES = [(1, 128, 64), (7, 136, 72), (16, 4864, 896), (33, 264, 200), (100, 1160, 328),
+          (128, 4864, 896), (129, 264, 200), (300, 1160, 328), (513, 392, 1096), (2560, 1032, 72)]
+
+
+@pytest.mark.parametrize("variant", [-1, 0, 1, 2, 3])
+@pytest.mark.parametrize("M,N,K", SHAPES)
+def test_packed_fused_every_variant(variant, M, N, K):
+    if variant == 2 and M > 128:
+        pytest.skip("small-M variant handles M <= 128")
+    A, W1, W2 = inputs.make_case(M, N, K, seed=1100 + M + N + K, std=0.05)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+    Wp = pack(W1, W2)
+    dA = dev(A)
+    dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+    B.swiglu_glu_mlp_packed(dA, Wp, dY, "silu", variant)
+    torch.cuda.synchronize()
+    assert_parity(host(dY), y_ref, ("packed", variant, M, N, K))
+    if variant == -1:
+        dY2 = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+        B.swiglu_mlp_packed(dA, Wp, dY2)
+        torch.cuda.synchronize()
+        assert np.array_equal(host(dY), host(dY2))
+
+
+@pytest.mark.parametrize("ksplit", [1, 2, 3, 5, 8])
+def test_packed_small_m_every_cluster_size(ksplit, monkeypatch):
+    monkeypatch.setenv("SWIGLU_KSPLIT", str(ksplit))
+    B.swiglu_reload_env()
+    try:
+        for M in (1, 16, 40, 128):
+            A, W1, W2 = inputs.make_case(M, 520, 712, seed=1200 + M, std=0.05)
+            y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+            dY = torch.full((M, 520), float("nan"), dtype=torch.bfloat16, device="cuda")
+            B.swiglu_glu_mlp_packed(dev(A), pack(W1, W2), dY, "silu", 2)
+            torch.cuda.synchronize()
+            assert_parity(host(dY), y_ref, ("packed smallm", M, ksplit))
+    finally:
+        monkeypatch.delenv("SWIGLU_KSPLIT")
+        B.swiglu_reload_env()
+
+
+@pytest.mark.parametrize("act", ["gelu", "gelu_tanh", "relu"])
+def test_packed_other_activations_and_nk_input(act):
+    K, N = 328, 1160
+    A_all, W1, W2 = inputs.make_case(300, N, K, seed=1300, std=0.1)
+    Wp = pack(W1, W2, B.WEIGHTS_NK)            # packed from the nn.Linear layout
+    for M in (9, 100, 300):
+        y_ref, _ = oracle.swiglu_oracle(A_all[:M], W1, W2, act=act)
+        dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+        B.swiglu_glu_mlp_packed(dev(A_all[:M]), Wp, dY, act)
+        torch.cuda.synchronize()
+        assert_parity(host(dY), y_ref, ("packed", act, M))
+
+
+def test_packed_baseline_shapes_sampled_rows():
+    """BASELINE.json shapes 0.5B and 7B at full size through the packed entry point, automatic
+    dispatch, every M of the config; bit-identical to the unpacked entry point where both run
+    the same kernel arithmetic (same tiles, same k order)."""
+    for shape in ("qwen2.5-0.5b", "qwen2.5-7b"):
+        K, N, seed, Ms = inputs.SHAPES[shape]
+        W1, W2 = inputs.make_weights(K, N, seed)
+        A_max = inputs.make_activations(max(Ms), K, seed)
+        dW1, dW2 = dev(W1), dev(W2)
+        Wp = pack(W1, W2)
+        for M in Ms:
+            rows = inputs.sample_rows(M)
+            if len(rows) > 64:
+                rows = rows[np.linspace(0, len(rows) - 1, 64).round().astype(int)]
+            y_ref, _ = oracle.swiglu_oracle_rows(A_max[:M], W1, W2, rows)
+            dA = dev(A_max[:M])
+            dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+            B.swiglu_mlp_packed(dA, Wp, dY)
+            dY2 = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+            B.swiglu_mlp(dA, dW1, dW2, dY2)
+            torch.cuda.synchronize()
+            rep = check.compare(host(dY[torch.from_numpy(rows).cuda()]), y_ref)
+            assert rep.mismatches == 0, (shape, M, rep)
+            assert bool(torch.isfinite(dY.float()).all())
+            assert np.array_equal(host(dY), host(dY2)), (shape, M)
+
+
+def test_packed_decode_chain_in_a_cuda_graph():
+    """A chain of dependent decode calls replayed from a CUDA graph: call i+1 loads its packed
+    weights before call i has finished (programmatic dependent launch) but reads the activations
+    call i wrote only after it has completed.  Y of one call is A of the next."""
+    M, K = 16, 512
+    N = K                                            # so that Y can feed the next call as A
+    A, W1, W2 = inputs.make_case(M, N, K, seed=1400, std=0.06)
+    Wp = pack(W1, W2)
+    bufs = [dev(A)] + [torch.zeros((M, N), dtype=torch.bfloat16, device="cuda") for _ in range(6)]
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        for i in range(6):
+            B.swiglu_mlp_packed(bufs[i], Wp, bufs[i + 1])
+    for _ in range(3):
+        g.replay()
+    torch.cuda.synchronize()
+    cur = A
+    for i in range(6):
+        y_ref, _ = oracle.swiglu_oracle(cur, W1, W2)
+        got = host(bufs[i + 1])
+        assert_parity(got, y_ref, ("chain", i))
+        cur = got                                   # the next call saw exactly these bf16 bits
+
+
+def test_launch_floor_probe_writes_nothing():
+    M, N, K = 16, 4864, 896
+    A, W1, W2 = inputs.make_case(M, N, K, seed=1500)
+    dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+    for _ in range(5):
+        B.swiglu_launch_floor_probe(dev(A), dev(W1), dev(W2), dY)
+    torch.cuda.synchronize()
+    assert bool(torch.isnan(dY.float()).all())
+    big = torch.zeros((300, N), dtype=torch.bfloat16, device="cuda")
+    bigA = torch.zeros((300, K), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(B.SwigluError) as e:
+        B.swiglu_launch_floor_probe(bigA, dev(W1), dev(W2), big)
+    assert e.value.status == B.SWIGLU_ERR_UNSUPPORTED
