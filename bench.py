@@ -231,6 +231,24 @@ class Workload:
             return lib.swiglu_mlp_unfused_ex(a, w1, w2, y, m, n, k, ws, need, -1, stream)
         return fn
 
+    def fused_fn(self, variant=-1):
+        """swiglu_mlp_ex with a caller-owned (zero-initialised) workspace: the timing loop replays
+        a captured CUDA graph, and under capture the library does not create its own K-split
+        workspace (include/swiglu_mlp.h) -- with the _ex form the captured calls run the same
+        schedule (K-split last wave) an eager swiglu_mlp call does."""
+        import torch
+        from paper_2607_02521_b200 import binding as B
+        lib = B.load()
+        need = max(int(lib.swiglu_workspace_bytes(m, self.N, self.K, 0, v)) for v in (0, 1) for m in self.Ms)
+        need = max(need, 256)
+        if getattr(self, "_fws", None) is None or self._fws.numel() < need:
+            self._fws = torch.zeros(need, dtype=torch.uint8, device="cuda")
+        ws, nbytes = self._fws.data_ptr(), self._fws.numel()
+
+        def fn(a, w1, w2, y, m, n, k, stream):
+            return lib.swiglu_mlp_ex(a, w1, w2, y, m, n, k, ws, nbytes, variant, stream)
+        return fn
+
     def flops_per_step(self):
         return sum(flops(M, self.N, self.K) for M in self.Ms)
 
@@ -369,7 +387,7 @@ def measure_points(wl, peaks, do_check=True, Ms=None, isolated=False):
     lib = B.load()
     pts = []
     for M in (Ms or wl.Ms):
-        f, u = time_points(wl, [lib.swiglu_mlp, wl.unfused_fn(M)], M)
+        f, u = time_points(wl, [wl.fused_fn(), wl.unfused_fn(M)], M)
         t = f["us_median"] * 1e-6
         fl, by = flops(M, wl.N, wl.K), algo_bytes(M, wl.N, wl.K)
         t_roof, bound = roofline_time_s(M, wl.N, wl.K, peaks["bf16_tflops"], peaks["hbm_gbs"])
@@ -807,9 +825,7 @@ def run_sweep(args):
         lines += ["| workload | M | " + " | ".join(f"S={k}" for k in ks) + " | auto (S) |", "|---|---|" + "---|" * 9]
 
     def forced(v):
-        def fn(a, w1, w2, y, M, N, K, stream):
-            return lib.swiglu_mlp_ex(a, w1, w2, y, M, N, K, None, 0, v, stream)
-        return fn
+        return lambda *a: forced.wl.fused_fn(v)(*a)
 
     def usable(fn, wl, M):
         try:
@@ -820,6 +836,7 @@ def run_sweep(args):
 
     for name in names:
         wl = Workload(name, Ms=Ms)
+        forced.wl = wl
         for M in Ms:
             if args.sweep == "variants":
                 # every variant of this (shape, M) sampled INTERLEAVED, so clock / power drift

@@ -11,9 +11,11 @@ from .oracle import (  # noqa: F401
     ACTIVATIONS,
     activation,
     build,
+    e4m3_to_f64,
     max_threads,
     pack_weights,
     silu,
     swiglu_oracle,
+    swiglu_oracle_fp8,
     swiglu_oracle_rows,
 )

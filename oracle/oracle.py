@@ -54,6 +54,11 @@ def _load():
         lib.swiglu_oracle_activation.restype = ctypes.c_double
         lib.swiglu_oracle_silu.argtypes = [ctypes.c_double]
         lib.swiglu_oracle_silu.restype = ctypes.c_double
+        lib.swiglu_oracle_e4m3_to_f64.argtypes = [ctypes.c_uint8]
+        lib.swiglu_oracle_e4m3_to_f64.restype = ctypes.c_double
+        lib.swiglu_oracle_fp8_rows.argtypes = [p, p, p, p, p, i64, i64, i64, i64, ctypes.c_double,
+                                               ctypes.c_double, ctypes.c_int]
+        lib.swiglu_oracle_fp8_rows.restype = ctypes.c_int
         lib.swiglu_oracle_pack.argtypes = [p, p, p, i64, i64]
         lib.swiglu_oracle_pack.restype = ctypes.c_int
         lib.swiglu_oracle_max_threads.argtypes = []
@@ -148,3 +153,32 @@ def pack_weights(W1_bits, W2_bits):
     if _load().swiglu_oracle_pack(_ptr(W1), _ptr(W2), _ptr(Wp), N, K) != 0:
         raise RuntimeError("swiglu_oracle_pack rejected its arguments")
     return Wp
+
+
+def e4m3_to_f64(code: int) -> float:
+    """The oracle's own decode of one OCP FP8 E4M3 code (for the pins)."""
+    return float(_load().swiglu_oracle_e4m3_to_f64(int(code) & 0xFF))
+
+
+def swiglu_oracle_fp8(A8, W1_8, W2_8, scale_gate=1.0, scale_up=1.0, rows=None, nthreads: int = 0):
+    """FP8 (E4M3) operands: y_ref = SiLU(scale_gate * A8.W1_8^T) * (scale_up * A8.W2_8^T) in fp64.
+    A8 [M,K], W1_8 / W2_8 [N,K] (K contiguous), all uint8 codes.  rows: optional row subset.
+    Returns (y_ref [len(rows) or M, N], threads_used)."""
+    A = np.ascontiguousarray(A8)
+    W1 = np.ascontiguousarray(W1_8)
+    W2 = np.ascontiguousarray(W2_8)
+    if A.dtype != np.uint8 or W1.dtype != np.uint8 or W2.dtype != np.uint8:
+        raise TypeError("FP8 operands are passed as uint8 codes")
+    M, K = A.shape
+    N, K2 = W1.shape
+    if K2 != K or W2.shape != (N, K):
+        raise ValueError(f"A is [{M},{K}] but W1 is {W1.shape}, W2 is {W2.shape} (need [N,K])")
+    r = None if rows is None else np.ascontiguousarray(np.asarray(rows, dtype=np.int64))
+    count = M if r is None else r.shape[0]
+    Y = np.empty((count, N), dtype=np.float64)
+    used = _load().swiglu_oracle_fp8_rows(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y),
+                                          None if r is None else _ptr(r), count, M, N, K,
+                                          float(scale_gate), float(scale_up), int(nthreads))
+    if used < 0:
+        raise RuntimeError("swiglu_oracle_fp8 rejected its arguments")
+    return Y, int(used)

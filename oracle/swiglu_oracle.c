@@ -201,6 +201,62 @@ int swiglu_oracle_rows(const uint16_t *A, const uint16_t *W1, const uint16_t *W2
 }
 
 /*
+ * FP8 operands ("FP8 ... we expect even larger relative gains"; line 392
+ * future-work item 2).  The paper gives no method detail, so the reading
+ * taken (R19) is the one FP8 serving stacks use: A and both weight matrices are
+ * OCP FP8 E4M3 ("e4m3fn": 1 sign, 4 exponent bits with bias 7, 3 mantissa bits, no infinities,
+ * S.1111.111 = NaN), weights in the [N, K] layout checkpoints store (K contiguous), one
+ * dequantisation scale per projection folded into two fp32 scalars:
+ *
+ *     Gate = scale_gate * (A8 . W1_8^T),  Up = scale_up * (A8 . W2_8^T),  Y = SiLU(Gate) (.) Up
+ *
+ * Same plain definition as above, fp64, k ascending; each product of two e4m3 values has an
+ * 8-bit significand and is exact.  The result is NOT rounded.
+ */
+double swiglu_oracle_e4m3_to_f64(uint8_t b) {
+  const int sign = b >> 7, e = (b >> 3) & 15, m = b & 7;
+  double v;
+  if (e == 15 && m == 7) return NAN;                 /* the only non-finite code (no inf) */
+  if (e == 0) v = ldexp((double)m / 8.0, -6);         /* subnormal: m/8 * 2^(1-7)           */
+  else v = ldexp(1.0 + (double)m / 8.0, e - 7);       /* normal: (1 + m/8) * 2^(e-7)        */
+  return sign ? -v : v;
+}
+
+/* rows[i] of Y for i < count (rows == NULL: row i itself); Ysub is [count, N] fp64. */
+int swiglu_oracle_fp8_rows(const uint8_t* A, const uint8_t* W1, const uint8_t* W2, double* Ysub,
+                           const int64_t* rows, int64_t count, int64_t M, int64_t N, int64_t K,
+                           double scale_gate, double scale_up, int nthreads) {
+  if (M < 0 || N < 0 || K < 0 || count < 0) return -1;
+  if (count == 0 || N == 0) return 0;
+  if ((!A || !W1 || !W2) && K > 0) return -1;
+  if (!Ysub) return -1;
+  for (int64_t i = 0; i < count; ++i) {
+    const int64_t m = rows ? rows[i] : i;
+    if (m < 0 || m >= M) return -1;
+  }
+  int used = 1;
+  const int64_t units = count * N;
+#ifdef _OPENMP
+  if (nthreads <= 0) nthreads = omp_get_max_threads();
+  if ((int64_t)nthreads > units) nthreads = (int)units;
+  used = nthreads;
+#pragma omp parallel for num_threads(nthreads) schedule(static)
+#endif
+  for (int64_t idx = 0; idx < units; ++idx) {        /* one output (row i, column n) at a time */
+    const int64_t i = idx / N, n = idx % N;
+    const int64_t m = rows ? rows[i] : i;
+    double gate = 0.0, up = 0.0;
+    for (int64_t k = 0; k < K; ++k) {                /* k ascending: the sums of Eq. 1, Eq. 2 */
+      const double a = swiglu_oracle_e4m3_to_f64(A[m * K + k]);
+      gate += a * swiglu_oracle_e4m3_to_f64(W1[n * K + k]);   /* W[n, k], row-major [N, K] */
+      up += a * swiglu_oracle_e4m3_to_f64(W2[n * K + k]);
+    }
+    Ysub[i * N + n] = swiglu_oracle_silu(scale_gate * gate) * (scale_up * up);   /* Eq. 3 */
+  }
+  return used;
+}
+
+/*
  * The one-time weight interleave ("W_fused"): Kernel-2
  * "interleaves W1 and W2" ahead of time so that a Gate column and its Up column reach the same
  * tile.  The paper does not print the layout; the reading taken (R18) interleaves

@@ -53,8 +53,13 @@ struct GemmParams {
   int m_tiles;   // ceil(M / (128*kCtaGroup))
   int n_tiles;   // ceil(N / (fused ? 128 : 256))
   int group_m;   // m-tiles per L2 raster group
-  int wide_tiles;   // tiles [0, wide_tiles) are full width; the rest are 64-column half tiles
-  int total_tiles;  // wide_tiles + 2 * (m_tiles*n_tiles - wide_tiles)
+  int wide_tiles;   // tiles [0, wide_tiles) are whole (full width, all of K); the rest -- the last
+                    // partial wave -- are cut into units: tail_ksplit K-ranges each (tail_ksplit
+                    // >= 2), or two 64-column half tiles (tail_ksplit == 0)
+  int total_tiles;  // schedule slots: wide_tiles + units of the cut tiles
+  int tail_ksplit;  // s: K-ranges per tile of the last wave (0 = no K split)
+  float* split_ws;  // [tail tile][CTA of the group][s][256 columns / 4][128 rows] float4 partials
+  int* split_ctr;   // [tail tile][CTA of the group] arrival counters, zero between launches
   int early_issue;      // 1: fill the ring before the CTA-wide setup barrier (small grids)
   int w_evict_first;    // 1: weights are read once (one row of tiles): L2 evict-first loads
   unsigned long long* clk;  // optional {SM cycles, globaltimer ns} of CTA 0 (swiglu_set_clock_probe)
@@ -118,6 +123,34 @@ __device__ __forceinline__ void decode_tile_w(const GemmParams& p, int t, int& t
     n_base = tn * kOutCols + (j & 1) * 64;
     w = 64;
   }
+}
+
+// One schedule slot: which tile, which columns, which k-blocks.  tail >= 0: a K-range unit of
+// tail tile `tail` (rank `krank` of p.tail_ksplit), whose fp32 partial accumulators are combined
+// through p.split_ws by the last unit of that tile to arrive (a1: the stream-K treatment of the
+// last partial wave -- idle CTA groups take K-ranges of the tail tiles
+// discuss the wave quantisation this removes).
+struct TileUnit {
+  int tm, n_base, w, kb0, kb1, tail, krank;
+};
+template <int kOutCols>
+__device__ __forceinline__ TileUnit decode_unit(const GemmParams& p, int t, int k_blocks) {
+  TileUnit u;
+  u.kb0 = 0; u.kb1 = k_blocks; u.tail = -1; u.krank = 0;
+  if (t >= p.wide_tiles && p.tail_ksplit >= 2) {
+    const int idx = t - p.wide_tiles;
+    u.tail = idx / p.tail_ksplit;
+    u.krank = idx - u.tail * p.tail_ksplit;
+    int tn;
+    decode_tile(p, p.wide_tiles + u.tail, u.tm, tn);
+    u.n_base = tn * kOutCols;
+    u.w = kOutCols;
+    u.kb0 = (int)(((long long)k_blocks * u.krank) / p.tail_ksplit);
+    u.kb1 = (int)(((long long)k_blocks * (u.krank + 1)) / p.tail_ksplit);
+  } else {
+    decode_tile_w<kOutCols>(p, t, u.tm, u.n_base, u.w);
+  }
+  return u;
 }
 
 // Gate activations of the GLU family (include/swiglu_mlp.h swiglu_activation; PAPER.md line 56
@@ -300,7 +333,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       if (lane == 0) {
         // The producer needs only the barriers it has just initialised: fill the ring before
         // the CTA-wide setup barrier so TMEM allocation overlaps the first loads' latency.
-        if (p.early_issue && group_id < total_tiles) {
+        if (p.early_issue && group_id < total_tiles) {  // (host: never with a K-split tail)
           pdl_wait_prior_grid();
           int tm, n_base, w;
           decode_tile_w<kOutCols>(p, group_id, tm, n_base, w);
@@ -328,12 +361,11 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     int s = (pre == kStages) ? 0 : pre;
     uint32_t ph = (pre == kStages) ? 1u : 0u;
     for (int t = group_id; t < total_tiles; t += num_groups) {
-      int tm, n_base, w;
-      decode_tile_w<kOutCols>(p, t, tm, n_base, w);
-      const int m_base = (tm * kCtaGroup + (int)rank) * BM;
-      for (int kb = (t == group_id) ? pre : 0; kb < k_blocks; ++kb) {
+      const TileUnit u = decode_unit<kOutCols>(p, t, k_blocks);
+      const int m_base = (u.tm * kCtaGroup + (int)rank) * BM;
+      for (int kb = (t == group_id) ? u.kb0 + pre : u.kb0; kb < u.kb1; ++kb) {
         mbar_wait(empty_bar(s), ph ^ 1u);
-        issue_loads(s, kb, m_base, n_base, w);
+        issue_loads(s, kb, m_base, u.n_base, u.w);
         if (++s == kStages) { s = 0; ph ^= 1u; }
       }
     }
@@ -353,10 +385,11 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       tcgen05_fence_after();
       const uint32_t d_tmem = tmem_base + as * UMMA_N;
       // half tiles of the last wave (Gate 64 | Up 64) use an N = 128 instruction
-      const uint32_t idesc = (kFused && kBN == 128 && t >= p.wide_tiles) ? idesc_half : idesc_full;
-      for (int kb = 0; kb < k_blocks; ++kb) {
+      const TileUnit u = decode_unit<kOutCols>(p, t, k_blocks);
+      const uint32_t idesc = (kFused && kBN == 128 && u.w == 64) ? idesc_half : idesc_full;
+      for (int kb = u.kb0; kb < u.kb1; ++kb) {
         mbar_wait(full_bar(s), ph);
-        if (kb == 0) SWIGLU_GEMM_TRACE(8 + it * 8 + 1);
+        if (kb == u.kb0) SWIGLU_GEMM_TRACE(8 + it * 8 + 1);
         tcgen05_fence_after();
         const uint32_t sa = smem_a(s), sb = smem_b(s);
 #pragma unroll
@@ -367,7 +400,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           // B, [N,K] weights: K-major like A (slabs of 64 n-rows are 8 KB = 8 groups of 8 rows).
           const uint64_t bdesc = kWK ? smem_desc_sw128(sb + k * (UMMA_K * 2), 16, 1024)
                                      : smem_desc_sw128(sb + k * (UMMA_K * 128), 8192, 1024);
-          umma_bf16<kCtaGroup>(d_tmem, adesc, bdesc, idesc, (kb | k) != 0 ? 1u : 0u);
+          umma_bf16<kCtaGroup>(d_tmem, adesc, bdesc, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
         }
         umma_commit<kCtaGroup>(empty_bar(s));  // smem stage free once these MMAs retire
         if (++s == kStages) { s = 0; ph ^= 1u; }
@@ -383,10 +416,11 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     const uint32_t leader_acc_empty0 = (kCtaGroup == 2) ? mapa_shared(acc_empty_bar(0), 0) : 0u;
     int it = 0;
     uint32_t chunk_ctr = 0;
+    const uint32_t ticket_slot = tmem_slot + 4u;
     for (int t = group_id; t < total_tiles; t += num_groups, ++it) {
-      int tm, n_base, w;
-      decode_tile_w<kOutCols>(p, t, tm, n_base, w);
-      const int m_base = (tm * kCtaGroup + (int)rank) * BM;
+      const TileUnit tu = decode_unit<kOutCols>(p, t, k_blocks);
+      const int n_base = tu.n_base, w = tu.w;
+      const int m_base = (tu.tm * kCtaGroup + (int)rank) * BM;
       const int chunks = kFused ? w / 64 : kChunks;  // 64-column chunks in this tile
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1u;
@@ -394,6 +428,48 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       if (issuer) SWIGLU_GEMM_TRACE(8 + it * 8 + 3);
       tcgen05_fence_after();
       const uint32_t tacc = tmem_base + ((q * 32u) << 16) + as * UMMA_N;
+      // K-range unit of a tail tile: park the fp32 partial accumulators in the workspace
+      // ([column/4][row] float4: a warp writes 512 contiguous bytes), then the LAST unit of the
+      // tile to arrive sums all partials in k-range order (fixed order: bitwise deterministic
+      // whoever is last) and runs the normal activation / store epilogue on the sums.
+      const float4* split_src = nullptr;
+      if constexpr (kFused && kBN == 128) {
+        if (tu.tail >= 0) {
+          const int S = p.tail_ksplit;
+          const size_t slot = (size_t)tu.tail * kCtaGroup + rank;
+          float4* part = reinterpret_cast<float4*>(p.split_ws) + (slot * S + tu.krank) * (size_t)(64 * BM);
+#pragma unroll 1
+          for (int cc = 0; cc < UMMA_N / 32; ++cc) {
+            uint32_t v[32];
+            tmem_ld_32x32b_x32(tacc + cc * 32, v);
+            tmem_ld_wait();
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+              part[(size_t)(cc * 8 + j) * BM + row] =
+                  make_float4(__uint_as_float(v[4 * j]), __uint_as_float(v[4 * j + 1]),
+                              __uint_as_float(v[4 * j + 2]), __uint_as_float(v[4 * j + 3]));
+          }
+          tcgen05_fence_before();
+          __syncwarp();
+          if (lane == 0) {  // TMEM stage drained
+            if constexpr (kCtaGroup == 2) mbar_arrive_cluster(leader_acc_empty0 + 8u * as);
+            else mbar_arrive(acc_empty_bar(as));
+          }
+          __threadfence();  // partials visible device-wide before the arrival is counted
+          named_bar_sync(1, kEpiWarps * 32);
+          if (issuer) {
+            const int ticket = atomicAdd(p.split_ctr + slot, 1);
+            if (ticket == S - 1) p.split_ctr[slot] = 0;  // all S arrived: clean for the next launch
+            __threadfence();
+            asm volatile("st.shared.b32 [%0], %1;" ::"r"(ticket_slot), "r"(ticket) : "memory");
+          }
+          named_bar_sync(1, kEpiWarps * 32);
+          int ticket;
+          asm volatile("ld.shared.b32 %0, [%1];" : "=r"(ticket) : "r"(ticket_slot) : "memory");
+          if (ticket != S - 1) continue;  // a later unit will finish this tile
+          split_src = reinterpret_cast<const float4*>(p.split_ws) + slot * S * (size_t)(64 * BM);
+        }
+      }
 #pragma unroll 1
       for (int h = 0; h < chunks; ++h, ++chunk_ctr) {
         const uint32_t obuf = smem_out + (chunk_ctr & 1u) * kOutBufBytes;
@@ -408,9 +484,33 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
             // accumulator columns: [Gate w | Up w], or g0 u0 g1 u1 for packed weights
             const uint32_t gcol = kPacked ? h * 128 + c * 32 : h * 64 + c * 32;
             const uint32_t ucol = kPacked ? gcol + 64 : gcol + w;
-            tmem_ld_32x32b_x32(tacc + gcol, g);
-            tmem_ld_32x32b_x32(tacc + ucol, u);
-            tmem_ld_wait();
+            if (kBN == 128 && split_src != nullptr) {
+              // sums of the K-range partials, k-range 0 first
+              float gs[32], us[32];
+#pragma unroll
+              for (int j = 0; j < 32; ++j) gs[j] = us[j] = 0.0f;
+#pragma unroll 1
+              for (int r = 0; r < p.tail_ksplit; ++r) {
+                const float4* pr = split_src + (size_t)r * (64 * BM) + row;
+                float4 a[8], b[8];  // 16 loads in flight per thread, then the adds in k-range order
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                  a[j] = __ldcg(pr + (size_t)(gcol / 4 + j) * BM);
+                  b[j] = __ldcg(pr + (size_t)(ucol / 4 + j) * BM);
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                  gs[4 * j] += a[j].x; gs[4 * j + 1] += a[j].y; gs[4 * j + 2] += a[j].z; gs[4 * j + 3] += a[j].w;
+                  us[4 * j] += b[j].x; us[4 * j + 1] += b[j].y; us[4 * j + 2] += b[j].z; us[4 * j + 3] += b[j].w;
+                }
+              }
+#pragma unroll
+              for (int j = 0; j < 32; ++j) { g[j] = __float_as_uint(gs[j]); u[j] = __float_as_uint(us[j]); }
+            } else {
+              tmem_ld_32x32b_x32(tacc + gcol, g);
+              tmem_ld_32x32b_x32(tacc + ucol, u);
+              tmem_ld_wait();
+            }
 #pragma unroll
             for (int j = 0; j < 16; ++j) {
               const float y0 =
@@ -427,7 +527,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
             for (int j = 0; j < 16; ++j)
               packed[j] = pack_bf16x2_rn(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
           }
-          if (h == chunks - 1 && c == 1) {
+          if (h == chunks - 1 && c == 1 && split_src == nullptr) {
             // last TMEM read of this tile is done: hand the accumulator stage back to the MMA
             tcgen05_fence_before();
             __syncwarp();

@@ -78,9 +78,9 @@ int env_int(const char* name, int dflt) {
 // first call into the library (and again only on swiglu_reload_env()): the hot path does no
 // getenv.  All default to "off" / "automatic".
 struct Env {
-  int variant = -1, unfused_variant = -1, ksplit = 0, group_m = 0, host_chunks = 4;
+  int variant = -1, unfused_variant = -1, ksplit = 0, group_m = 0, host_chunks = 4, tail_ksplit = 0;
   bool no_pdl = false, no_prefetch = false, no_early = false, no_tail_split = false,
-       no_w_evict_first = false, no_tmap_cache = false;
+       no_tail_ksplit = false, no_w_evict_first = false, no_tmap_cache = false;
 };
 Env g_env;
 std::once_flag g_env_once;
@@ -90,12 +90,15 @@ void load_env() {
   e.unfused_variant = env_int("SWIGLU_UNFUSED_VARIANT", -1);
   e.ksplit = env_int("SWIGLU_KSPLIT", 0);
   e.group_m = env_int("SWIGLU_GROUP_M", 0);
+  e.tail_ksplit = env_int("SWIGLU_TAIL_KSPLIT", 0);
+  if (e.tail_ksplit > 8) e.tail_ksplit = 8;
   e.host_chunks = env_int("SWIGLU_HOST_CHUNKS", 4);
   if (e.host_chunks <= 0) e.host_chunks = 4;
   e.no_pdl = env_int("SWIGLU_NO_PDL", 0) != 0;
   e.no_prefetch = env_int("SWIGLU_NO_PREFETCH", 0) != 0;
   e.no_early = env_int("SWIGLU_NO_EARLY", 0) != 0;
   e.no_tail_split = env_int("SWIGLU_NO_TAIL_SPLIT", 0) != 0;
+  e.no_tail_ksplit = env_int("SWIGLU_NO_TAIL_KSPLIT", 0) != 0;
   e.no_w_evict_first = env_int("SWIGLU_NO_W_EVICT_FIRST", 0) != 0;
   e.no_tmap_cache = env_int("SWIGLU_NO_TMAP_CACHE", 0) != 0;
   g_env = e;
@@ -179,6 +182,7 @@ struct DeviceState {
   struct Buf { void* ptr = nullptr; size_t bytes = 0; };
   std::map<cudaStream_t, Buf> workspace;     // unfused path: bf16 Gate | Up
   std::map<cudaStream_t, Buf> host_scratch;  // swiglu_mlp_host: device copies of A, W1, W2, Y
+  std::map<cudaStream_t, Buf> split_ws;      // fused large-M: K-split partials of the last wave
   // swiglu_mlp_host_batched: copy streams and events of its H2D / compute / D2H pipeline;
   // host_mu admits one such pipeline per device at a time
   std::mutex host_mu;
@@ -323,10 +327,45 @@ inline int64_t packed_slabs(int64_t N) { return 4 * ((N + 127) / 128); }
 
 bool pdl_enabled() { return !env().no_pdl; }
 
+// ------------------------------------------------------------------ last-wave plan (a1)
+// The last partial wave of a 128-column fused schedule (rem tiles on G CTA groups):
+//  * K split ("stream-K tail"): each tail tile is cut into s K-ranges run by otherwise idle
+//    groups; partial fp32 accumulators meet in a global workspace and the last range to arrive
+//    finishes the tile.  The finisher alone moves s x 128 KB per CTA through L2 (measured
+//    ~2 us per partial, profiles/r02_tail_ksplit.md), so the split pays only when half tiles
+//    would leave most of the machine idle (4 rem <= G) and every range keeps >= 16 k-blocks of
+//    mainloop: the big-K shapes near the ridge (72B at M = 256, 512).  s <= 4.
+//  * else, if at most half of the groups would be busy: two 64-column half tiles per tile.
+constexpr int kSplitMaxS = 4;
+constexpr int kSplitMinKBlocks = 16;
+constexpr size_t kSplitCtrBytes = 4096;                      // counters: one int per (tile, CTA)
+constexpr size_t kSplitPartialBytes = 256 * 128 * 4;         // one CTA's fp32 accumulators
+constexpr size_t kSplitWsBytes = kSplitCtrBytes + 160 * kSplitPartialBytes;  // up to 160 SMs
+struct TailPlan { int64_t wide, total; int ksplit; };
+TailPlan plan_tail(int64_t tiles, int G, int64_t k_blocks, bool fused128, bool have_ws) {
+  TailPlan t{tiles, tiles, 0};
+  const int64_t rem = tiles % G;
+  if (!fused128 || rem == 0 || env().no_tail_split) return t;
+  int s = (int)(G / rem);
+  if (s > kSplitMaxS) s = kSplitMaxS;
+  if (env().tail_ksplit > 0) s = env().tail_ksplit;   // experiments: force s (if it fits)
+  while (s >= 2 && (rem * s > G || k_blocks / s < (env().tail_ksplit > 0 ? 1 : kSplitMinKBlocks))) --s;
+  const bool sparse_tail = 4 * rem <= G || env().tail_ksplit > 0;
+  if (have_ws && s >= 2 && sparse_tail && !env().no_tail_ksplit) {
+    t.wide = tiles - rem;
+    t.ksplit = s;
+    t.total = t.wide + rem * s;
+  } else if (tiles > G && 2 * rem <= G) {
+    t.wide = tiles - rem;
+    t.total = tiles + rem;
+  }
+  return t;
+}
+
 // ------------------------------------------------------------------ launches
 template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = swiglu::kActSilu, int kWMode = 0>
 int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void* B2, void* Yout,
-                int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
+                int64_t M, int64_t N, int64_t K, cudaStream_t stream, void* split_ws = nullptr) {
   using namespace swiglu;
   CUtensorMap ta, tb1, tb2, ty;
   int rc;
@@ -359,21 +398,17 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   if (gm > p.m_tiles) gm = p.m_tiles;
   p.group_m = (int)gm;
   const int64_t tiles = (int64_t)p.m_tiles * p.n_tiles;
-  int groups = d.sm_count / kCtaGroup;
-  if (tiles < groups) groups = (int)tiles;
-  // Last partial wave: if at most half of the CTA groups would get a tile, cut those tiles into
-  // 64-column halves so the wave takes half a tile time on all SMs (fused 128-column tiles only).
-  p.wide_tiles = (int)tiles;
-  p.total_tiles = (int)tiles;
-  if (kFused && kBN == 128 && tiles > groups && !env().no_tail_split) {
-    const int64_t rem = tiles % groups;
-    if (rem > 0 && 2 * rem <= groups) {
-      p.wide_tiles = (int)(tiles - rem);
-      p.total_tiles = (int)(tiles + rem);
-    }
-  }
+  const int G = d.sm_count / kCtaGroup;
+  const TailPlan tail = plan_tail(tiles, G, (K + BK - 1) / BK, kFused && kBN == 128,
+                                  split_ws != nullptr && d.sm_count <= 160);
+  p.wide_tiles = (int)tail.wide;
+  p.total_tiles = (int)tail.total;
+  p.tail_ksplit = tail.ksplit;
+  p.split_ctr = (int*)split_ws;
+  p.split_ws = split_ws ? (float*)((char*)split_ws + kSplitCtrBytes) : nullptr;
+  const int groups = (int)(tail.total < G ? tail.total : G);
   // one tile per CTA (a short, HBM-bound call): fill the TMA ring before the setup barrier
-  p.early_issue = (kCtaGroup == 1 && kFused && tiles <= groups && !env().no_early);
+  p.early_issue = (kCtaGroup == 1 && kFused && tiles <= groups && tail.ksplit == 0 && !env().no_early);
   p.w_evict_first = (p.m_tiles == 1 && !env().no_w_evict_first);
   p.clk = g_clk.load(std::memory_order_relaxed);
 #ifdef SWIGLU_TRACE
@@ -545,8 +580,15 @@ size_t workspace_for(int64_t M, int64_t N, int64_t K, int unfused, int variant) 
   if (M <= 0 || N <= 0 || K <= 0) return 0;
   if (unfused) return 2 * round_up((size_t)M * N * 2, 256);  // Gate and Up, bf16
   if (variant < 0) variant = select_fused(M, N, K);
-  (void)variant;
-  return 0;  // fused variants reduce split-K partials on chip (DSMEM), no global workspace
+  // The 128-column large-M kernels can cut their last partial wave in K through a workspace
+  // (optional: without it they fall back to 64-column half tiles).  Sized for 148 SMs here --
+  // this query makes no CUDA call.  The decode kernel reduces on chip (DSMEM): no workspace.
+  if (variant == kFused1Cta || variant == kFused2Cta) {
+    const int cg = variant == kFused2Cta ? 2 : 1;
+    const int64_t tiles = ((M + 128 * cg - 1) / (128 * cg)) * ((N + 127) / 128);
+    if (plan_tail(tiles, 148 / cg, (K + 63) / 64, true, true).ksplit >= 2) return kSplitWsBytes;
+  }
+  return 0;
 }
 
 // Library-owned buffer of `stream` in `pool`, at least `need` bytes.  Allocation and growth are
@@ -595,10 +637,11 @@ int release_pool(std::map<cudaStream_t, DeviceState::Buf>& pool, bool all, cudaS
 
 template <int kAct, int kWK>
 int launch_fused_l(const DeviceState& d, int variant, const void* A, const void* W1,
-                   const void* W2, void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
+                   const void* W2, void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream,
+                   void* split_ws) {
   switch (variant) {
-    case kFused1Cta: return launch_gemm<1, true, 128, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
-    case kFused2Cta: return launch_gemm<2, true, 128, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
+    case kFused1Cta: return launch_gemm<1, true, 128, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream, split_ws);
+    case kFused2Cta: return launch_gemm<2, true, 128, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream, split_ws);
     case kFusedSmallM: return launch_smallm<kAct, kWK>(d, A, W1, W2, Y, nullptr, M, N, K, stream);
     case kFused1CtaN64: return launch_gemm<1, true, 64, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
   }
@@ -606,17 +649,43 @@ int launch_fused_l(const DeviceState& d, int variant, const void* A, const void*
 }
 template <int kAct>
 int launch_fused(const DeviceState& d, int variant, int layout, const void* A, const void* W1,
-                 const void* W2, void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream) {
+                 const void* W2, void* Y, int64_t M, int64_t N, int64_t K, cudaStream_t stream,
+                 void* split_ws) {
   switch (layout) {
-    case kWeightsNK: return launch_fused_l<kAct, kWeightsNK>(d, variant, A, W1, W2, Y, M, N, K, stream);
-    case kWeightsPacked: return launch_fused_l<kAct, kWeightsPacked>(d, variant, A, W1, W2, Y, M, N, K, stream);
+    case kWeightsNK: return launch_fused_l<kAct, kWeightsNK>(d, variant, A, W1, W2, Y, M, N, K, stream, split_ws);
+    case kWeightsPacked: return launch_fused_l<kAct, kWeightsPacked>(d, variant, A, W1, W2, Y, M, N, K, stream, split_ws);
   }
-  return launch_fused_l<kAct, kWeightsKN>(d, variant, A, W1, W2, Y, M, N, K, stream);
+  return launch_fused_l<kAct, kWeightsKN>(d, variant, A, W1, W2, Y, M, N, K, stream, split_ws);
+}
+
+// Library-owned K-split workspace of `stream`: FIXED size (never regrown, so a captured graph's
+// pointer stays valid until swiglu_release), counters zeroed once in stream order.  Not created
+// while the stream is capturing: the caller then gets no K split (half tiles instead) unless it
+// passes its own workspace through the _ex form.
+void* split_workspace(DeviceState& d, cudaStream_t stream) {
+  std::lock_guard<std::mutex> lk(g_mu);
+  auto it = d.split_ws.find(stream);
+  if (it != d.split_ws.end()) return it->second.ptr;
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(stream, &cap);
+  if (cap != cudaStreamCaptureStatusNone) return nullptr;
+  void* ptr = nullptr;
+  if (cudaMallocAsync(&ptr, kSplitWsBytes, stream) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  if (cudaMemsetAsync(ptr, 0, kSplitCtrBytes, stream) != cudaSuccess) {
+    cudaGetLastError();
+    cudaFreeAsync(ptr, stream);
+    return nullptr;
+  }
+  d.split_ws[stream] = DeviceState::Buf{ptr, kSplitWsBytes};
+  return ptr;
 }
 
 // layout: SWIGLU_WEIGHTS_KN / _NK, or kWeightsPacked (internal: W1 = W2 = the packed buffer).
+// ws / own_ws: the optional K-split workspace (see plan_tail): the caller's (own_ws == false; used
+// if it is large enough, ignored otherwise) or the library's per-stream one.
 int run_fused(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
-              int64_t K, int variant, int act, int layout, cudaStream_t stream) {
+              int64_t K, int variant, int act, int layout, cudaStream_t stream,
+              void* ws = nullptr, size_t ws_bytes = 0, bool own_ws = true) {
   if (layout != SWIGLU_WEIGHTS_KN && layout != SWIGLU_WEIGHTS_NK && layout != kWeightsPacked)
     return fail(SWIGLU_ERR_UNSUPPORTED, "unknown weight layout %d", layout);
   int rc = validate(A, W1, W2, Y, M, N, K);
@@ -637,12 +706,17 @@ int run_fused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
   DeviceState* d;
   if ((rc = get_device_state(&d))) return rc;
   if (variant < 0) variant = select_fused(M, N, K);
+  void* split_ws = nullptr;
+  if (workspace_for(M, N, K, 0, variant) > 0) {
+    if (own_ws) split_ws = split_workspace(*d, stream);
+    else if (ws && ws_bytes >= kSplitWsBytes && !((uintptr_t)ws & 255u)) split_ws = ws;
+  }
   using namespace swiglu;
   switch (act) {
-    case kActSilu: return launch_fused<kActSilu>(*d, variant, layout, A, W1, W2, Y, M, N, K, stream);
-    case kActGelu: return launch_fused<kActGelu>(*d, variant, layout, A, W1, W2, Y, M, N, K, stream);
-    case kActGeluTanh: return launch_fused<kActGeluTanh>(*d, variant, layout, A, W1, W2, Y, M, N, K, stream);
-    case kActRelu: return launch_fused<kActRelu>(*d, variant, layout, A, W1, W2, Y, M, N, K, stream);
+    case kActSilu: return launch_fused<kActSilu>(*d, variant, layout, A, W1, W2, Y, M, N, K, stream, split_ws);
+    case kActGelu: return launch_fused<kActGelu>(*d, variant, layout, A, W1, W2, Y, M, N, K, stream, split_ws);
+    case kActGeluTanh: return launch_fused<kActGeluTanh>(*d, variant, layout, A, W1, W2, Y, M, N, K, stream, split_ws);
+    case kActRelu: return launch_fused<kActRelu>(*d, variant, layout, A, W1, W2, Y, M, N, K, stream, split_ws);
   }
   return fail(SWIGLU_ERR_UNSUPPORTED, "unknown activation %d", act);
 }
@@ -712,8 +786,9 @@ int swiglu_mlp(const void* A, const void* W1, const void* W2, void* Y, int64_t M
 int swiglu_mlp_ex(const void* A, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
                   int64_t K, void* workspace, size_t workspace_bytes, int variant,
                   void* stream) {
-  (void)workspace; (void)workspace_bytes;  // no fused variant needs a global workspace
-  return run_fused(A, W1, W2, Y, M, N, K, variant, swiglu::kActSilu, 0, (cudaStream_t)stream);
+  // optional: only the K split of the last wave uses it (swiglu_workspace_bytes says when)
+  return run_fused(A, W1, W2, Y, M, N, K, variant, swiglu::kActSilu, 0, (cudaStream_t)stream,
+                   workspace, workspace_bytes, false);
 }
 
 int swiglu_mlp_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
@@ -1034,6 +1109,7 @@ int swiglu_release_stream(void* stream_v) {
   DeviceState& d = g_dev[dev];
   int rc;
   if ((rc = release_pool(d.workspace, false, stream))) return rc;
+  if ((rc = release_pool(d.split_ws, false, stream))) return rc;
   return release_pool(d.host_scratch, false, stream);
 }
 
@@ -1047,6 +1123,7 @@ int swiglu_release(void) {
   std::lock_guard<std::mutex> lk(g_mu);
   int rc;
   if ((rc = release_pool(d.workspace, true, nullptr))) return rc;
+  if ((rc = release_pool(d.split_ws, true, nullptr))) return rc;
   if ((rc = release_pool(d.host_scratch, true, nullptr))) return rc;
   if (d.s_in) {
     cudaStreamDestroy(d.s_in);

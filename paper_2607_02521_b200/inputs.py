@@ -95,3 +95,39 @@ def sample_rows(M: int, per_tile: int = 8, tile: int = 128):
     offs = (0, 31, 32, 63, 64, 95, 96, 127)[:per_tile]
     rows = sorted({t + o for t in range(0, M, tile) for o in offs if t + o < M} | {M - 1})
     return np.asarray(rows, dtype=np.int64)
+
+
+# ---------------------------------------------------------------------------------------
+# FP8 (OCP E4M3, "e4m3fn") inputs for the FP8-operand entry point.
+# Input preparation only: quantising random numbers to the format the call consumes.
+# ---------------------------------------------------------------------------------------
+def _e4m3_magnitudes() -> np.ndarray:
+    """The 127 finite non-negative E4M3 values in code order (code = index)."""
+    code = np.arange(127)
+    e, m = code >> 3, code & 7
+    return np.where(e == 0, (m / 8.0) * 2.0 ** -6, (1.0 + m / 8.0) * 2.0 ** (e.astype(np.float64) - 7))
+
+
+def f32_to_e4m3_bits(x: np.ndarray) -> np.ndarray:
+    """fp32 -> E4M3 code (uint8): round to nearest, ties to the even code, saturating at +-448."""
+    x = np.ascontiguousarray(x, dtype=np.float32).astype(np.float64)
+    mags = _e4m3_magnitudes()
+    mids = (mags[:-1] + mags[1:]) / 2.0
+    a = np.abs(x)
+    idx = np.searchsorted(mids, a, side="left")               # midpoints strictly below |x|
+    tie = (idx < mids.size) & (a == mids[np.minimum(idx, mids.size - 1)])
+    idx = np.where(tie & (idx % 2 == 1), idx + 1, idx)        # exact tie: take the even code
+    idx = np.minimum(idx, 126).astype(np.uint8)               # saturate to 448
+    return (idx | (np.signbit(x).astype(np.uint8) << 7)).astype(np.uint8)
+
+
+def make_fp8_case(M: int, N: int, K: int, seed: int, std: float = W_STD):
+    """(A8 [M,K], W1_8 [N,K], W2_8 [N,K], scale_gate, scale_up): A ~ N(0,1) quantised directly;
+    W ~ N(0, std) quantised as W / std (so the codes span the format) with dequantisation scale
+    std folded into scale_gate = scale_up = std.  Weights in the [N,K] (nn.Linear) layout."""
+    gen = lambda key, count: np.random.Generator(np.random.Philox(key=int(key))).standard_normal(
+        count, dtype=np.float32)
+    a8 = f32_to_e4m3_bits(gen(4 * seed + 2, M * K)).reshape(M, K)
+    w1 = f32_to_e4m3_bits(gen(4 * seed + 0, N * K)).reshape(N, K)
+    w2 = f32_to_e4m3_bits(gen(4 * seed + 1, N * K)).reshape(N, K)
+    return a8, w1, w2, float(std), float(std)

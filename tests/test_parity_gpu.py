@@ -135,6 +135,63 @@ def test_last_wave_half_tiles(variant, M, N, K, swiglu_env):
     assert_parity(y_plain, y_ref, ("no-split", variant, M, N, K))
 
 
+@pytest.mark.parametrize("force_s", [0, 2, 3, 8])
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("M,N,K", [
+    (2560, 1024, 512),    # 1-CTA: 160 tiles -> 12 tail tiles; 2-CTA: 80 -> 6
+    (2305, 1160, 328),    # ragged M / N / K (K % 64 != 0), k-blocks not divisible by the split
+    (300, 4864, 896),     # a single partial wave on the 2-CTA kernel (76 pair tiles on 74 groups)
+    (512, 9472, 4096),    # 74 column tiles x 2-4 row tiles, 64 k-blocks: splits under the policy
+])
+def test_last_wave_k_split(variant, M, N, K, force_s, swiglu_env):
+    """a1, the stream-K treatment of the last partial wave: tail tiles are cut into K-ranges run
+    by otherwise idle CTA groups, partial sums meet in a workspace, the last range to arrive
+    finishes the tile.  force_s = 0: the library's own policy; otherwise SWIGLU_TAIL_KSPLIT
+    forces that many ranges (where they fit).  Library-owned workspace and caller workspace
+    (_ex) must agree bit for bit, be run-to-run deterministic, leave the counters at zero, and
+    match the half-tile and unsplit schedules within the bound."""
+    if force_s:
+        swiglu_env("SWIGLU_TAIL_KSPLIT", force_s)
+    A, W1, W2 = inputs.make_case(M, N, K, seed=450 + N + K, std=0.05)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+    dA, dW1, dW2 = dev(A), dev(W1), dev(W2)
+    need = B.swiglu_workspace_bytes(M, N, K, unfused=False, variant=variant)
+
+    def call(ws=None):
+        dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+        if ws is None:
+            B.swiglu_glu_mlp_ex(dA, dW1, dW2, dY, "silu", variant=variant)   # library workspace
+        else:
+            B.swiglu_mlp_ex(dA, dW1, dW2, dY, workspace=ws, workspace_bytes=ws.numel(), variant=variant)
+        torch.cuda.synchronize()
+        return host(dY)
+
+    y_lib = call()
+    assert_parity(y_lib, y_ref, ("k-split lib ws", variant, M, N, K, force_s))
+    if need:
+        ws = torch.zeros(need, dtype=torch.uint8, device="cuda")
+        for _ in range(3):                           # counters must come back to zero each time
+            assert np.array_equal(call(ws), y_lib)
+        assert int(ws[:4096].view(torch.int32).abs().sum()) == 0
+    assert np.array_equal(call(), y_lib)             # deterministic whoever arrives last
+    swiglu_env("SWIGLU_NO_TAIL_KSPLIT", 1)
+    assert_parity(call(), y_ref, ("half tiles", variant, M, N, K))
+    swiglu_env("SWIGLU_NO_TAIL_SPLIT", 1)
+    assert_parity(call(), y_ref, ("no split", variant, M, N, K))
+
+
+def test_k_split_is_planned_only_where_it_pays():
+    """Host-side plan: a sparse last wave of a big-K shape gets a workspace (= a
+    K split); full waves, dense tails and short K do not."""
+    ws = lambda M, N, K, v: B.swiglu_workspace_bytes(M, N, K, unfused=False, variant=v)
+    assert ws(256, 29568, 8192, 1) > 0       # 72B M=256: 231 pair tiles on 74 pairs -> 9 x 4
+    assert ws(512, 29568, 8192, 1) > 0       # 72B M=512: 462 -> 18 x 4
+    assert ws(256, 13824, 5120, 1) == 0      # 14B M=256: 34 tail tiles: half tiles fill the machine
+    assert ws(256, 18944, 3584, 1) == 0      # 7B M=256: 148 tiles = 2 full waves
+    assert ws(4096, 8960, 1536, 1) == 0      # 1.5B: 24 k-blocks are too few to split
+    assert ws(16, 4864, 896, -1) == 0        # decode kernel reduces on chip
+
+
 def test_small_m_variant_rejects_large_m():
     A, W1, W2 = inputs.make_case(129, 128, 64, seed=1)
     with pytest.raises(B.SwigluError) as e:
