@@ -803,6 +803,70 @@ def run_decode_study(args):
     open(os.path.join(ROOT, "gpurun_out", "decode_study.md"), "w").write("\n".join(lines) + "\n")
 
 
+def run_fp8(args):
+    """FP8-operand table (`--fp8`): per BASELINE.json (shape, M) the FP8
+    (E4M3) fused call next to the bf16 fused call on the same shape -- microseconds (cold L2,
+    CUDA-graph replay, interleaved sampling), TFLOP/s (4MNK), fraction of the FP8 roofline
+    max(4MNK / (2 x measured bf16 peak), (2KN + MK + 2MN bytes) / HBM) -- the guide's nominal
+    fp8 : bf16 = 2 ratio applied to the measured bf16 peak -- and mismatches against the fp64 FP8
+    oracle on sampled rows.  Writes gpurun_out/fp8_results.md."""
+    import numpy as np
+    import torch
+    import oracle
+    from paper_2607_02521_b200 import binding as B, check, inputs
+    lib = B.load()
+    peaks, peak_src = load_peaks()
+    names = [n for n in inputs.SHAPES if not args.only or n in args.only.split(",")]
+    lines = ["| workload | M | variant | fp8 us | fp8 TFLOP/s | fp8 GB/s | bound | % of fp8 roofline "
+             "(2 x measured bf16 peak) | SM MHz | bf16 fused us | fp8 speed-up over bf16 | "
+             "mismatches (checked) |", "|" + "---|" * 12]
+    for name in names:
+        wl = Workload(name)
+        K, N = wl.K, wl.N
+        A8h, W1h, W2h, sg, su = inputs.make_fp8_case(wl.Mmax, N, K, seed=50 + wl.seed)
+        wbytes = 2 * K * N
+        copies = 1 if wbytes >= 2 * L2_BYTES else -(-2 * L2_BYTES // wbytes) + 1
+        up = lambda x: torch.from_numpy(x).cuda()
+        A8 = [up(A8h) for _ in range(copies)]
+        W1 = [up(W1h) for _ in range(copies)]
+        W2 = [up(W2h) for _ in range(copies)]
+        ctr = [0]
+
+        def fp8(a, w1, w2, y, m, n, k, stream):
+            c = ctr[0] % copies
+            ctr[0] += 1
+            return lib.swiglu_mlp_fp8(A8[c].data_ptr(), W1[c].data_ptr(), W2[c].data_ptr(), y, m, n, k,
+                                      sg, su, stream)
+        for M in wl.Ms:
+            f8, f16 = time_points(wl, [fp8, wl.fused_fn()], M, batches=args.sweep_batches)
+            t = f8["us_median"] * 1e-6
+            fl = flops(M, N, K)
+            by = 2 * K * N + M * K + M * N * 2
+            tc, tm = fl / (2 * peaks["bf16_tflops"] * 1e12), by / (peaks["hbm_gbs"] * 1e9)
+            rows = inputs.sample_rows(M)
+            if len(rows) > 32:
+                rows = rows[np.linspace(0, len(rows) - 1, 32).round().astype(int)]
+            y_ref, _ = oracle.swiglu_oracle_fp8(A8h[:M], W1h, W2h, sg, su, rows=rows)
+            wl.Y[:M].fill_(float("nan"))
+            rc = lib.swiglu_mlp_fp8(A8[0].data_ptr(), W1[0].data_ptr(), W2[0].data_ptr(), wl.Y.data_ptr(),
+                                    M, N, K, sg, su, torch.cuda.current_stream().cuda_stream)
+            assert rc == 0, B.last_error()
+            torch.cuda.synchronize()
+            y = wl.Y[:M][torch.from_numpy(rows).cuda()].view(torch.int16).cpu().numpy().view(np.uint16)
+            rep = check.compare(y, y_ref)
+            lines.append(f"| {name} | {M} | {B.swiglu_variant_name(B.swiglu_selected_variant(M, N, K))} | "
+                         f"{f8['us_median']:.2f} | {fl / t / 1e12:.1f} | {by / t / 1e9:.0f} | "
+                         f"{'tensor' if tc >= tm else 'hbm'} | {100 * max(tc, tm) / t:.1f} | {f8['sm_mhz'] or '-'} | "
+                         f"{f16['us_median']:.2f} | {f16['us_median'] / f8['us_median']:.3f} | "
+                         f"{rep.mismatches} ({rep.checked}) |")
+            print(lines[-1], flush=True)
+        del wl, A8, W1, W2
+        torch.cuda.empty_cache()
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    open(os.path.join(ROOT, "gpurun_out", "fp8_results.md"), "w").write("\n".join(lines) + "\n")
+    print(json.dumps({"peak_source": peak_src, "fp8_peak_tflops": 2 * peaks["bf16_tflops"]}))
+
+
 def run_sweep(args):
     """Dispatch-table sweeps (`--sweep variants` / `--sweep ksplit`): time every fused variant
     (forced through swiglu_mlp_ex) or every split-K factor of the small-M kernel
@@ -887,6 +951,7 @@ def main():
     ap.add_argument("--sweep-m", default="1,16,32,64,128,256")
     ap.add_argument("--sweep-batches", type=int, default=15)
     ap.add_argument("--decode-study", action="store_true")
+    ap.add_argument("--fp8", action="store_true")
     args = ap.parse_args()
     from paper_2607_02521_b200.dist import Ranks
     if args.impl == "reference":
@@ -905,6 +970,9 @@ def main():
         return
     if args.decode_study:
         run_decode_study(args)
+        return
+    if args.fp8:
+        run_fp8(args)
         return
     ranks = Ranks()
     if ranks.world != args.gpus and ranks.rank == 0:

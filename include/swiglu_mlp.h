@@ -172,6 +172,32 @@ int swiglu_glu_mlp_packed(const void* A, const void* Wp, void* Y, int64_t M, int
                           int64_t K, int activation, int variant, void* stream);
 
 /*
+ * FP8 operands ("For FP8 ... we expect even larger relative gains since the
+ * elementwise overhead grows relative to the faster GEMMs"; line 392 future-work item 2;
+ * SURVEY.md 8(f) N5).  The paper gives no method detail; the contract taken (R19):
+ *
+ *     Y = bf16( SiLU(scale_gate * (A8 . W1_8^T)) * (scale_up * (A8 . W2_8^T)) )
+ *
+ *     A8   : M x K  OCP FP8 E4M3 ("e4m3fn") bytes, K contiguous        (device, 16-byte aligned)
+ *     W1_8 : N x K  E4M3 bytes, K contiguous -- the [N,K] layout FP8 checkpoints store
+ *     W2_8 : N x K  E4M3 bytes, K contiguous
+ *     Y    : M x N  bf16, N contiguous                                  (written)
+ *     scale_gate, scale_up : fp32 host scalars, the folded per-tensor dequantisation scales
+ *                            (s_A * s_W1 and s_A * s_W2)
+ *
+ * K must be a multiple of 16 and N of 8.  tcgen05.mma kind::f8f6f4, fp32 accumulation over all
+ * of K, scales / SiLU / product in fp32 on the accumulators, one RNE rounding to bf16; Gate and
+ * Up never exist in HBM.  Same dispatch, variants (`variant`, -1 = automatic) and error
+ * behaviour as swiglu_mlp_ex; SiLU only.  NaN codes (0x7F, 0xFF) in the inputs are out of
+ * contract.
+ */
+int swiglu_mlp_fp8(const void* A8, const void* W1_8, const void* W2_8, void* Y, int64_t M,
+                   int64_t N, int64_t K, float scale_gate, float scale_up, void* stream);
+int swiglu_mlp_fp8_ex(const void* A8, const void* W1_8, const void* W2_8, void* Y, int64_t M,
+                      int64_t N, int64_t K, float scale_gate, float scale_up, int variant,
+                      void* stream);
+
+/*
  * Launch-floor probe (measurement aid): enqueues the decode kernel that swiglu_mlp would pick
  * for this (M <= 128, N, K) -- same grid, cluster dimensions, shared memory, tensor-map
  * parameters, barrier initialisation, TMEM allocation and programmatic-dependent-launch

@@ -34,6 +34,7 @@ EXPORTS = (
     "swiglu_release", "swiglu_release_stream", "swiglu_reload_env", "swiglu_tensor_map_cache_stats",
     "swiglu_set_clock_probe", "swiglu_packed_weight_bytes", "swiglu_pack_weights",
     "swiglu_mlp_packed", "swiglu_glu_mlp_packed", "swiglu_launch_floor_probe",
+    "swiglu_mlp_fp8", "swiglu_mlp_fp8_ex",
 )
 
 
@@ -93,6 +94,10 @@ def load():
     lib.swiglu_mlp_packed.argtypes, lib.swiglu_mlp_packed.restype = [p, p, p, i64, i64, i64, p], ci
     lib.swiglu_glu_mlp_packed.argtypes = [p, p, p, i64, i64, i64, ci, ci, p]
     lib.swiglu_glu_mlp_packed.restype = ci
+    cf = ctypes.c_float
+    lib.swiglu_mlp_fp8.argtypes, lib.swiglu_mlp_fp8.restype = [p, p, p, p, i64, i64, i64, cf, cf, p], ci
+    lib.swiglu_mlp_fp8_ex.argtypes = [p, p, p, p, i64, i64, i64, cf, cf, ci, p]
+    lib.swiglu_mlp_fp8_ex.restype = ci
     lib.swiglu_launch_floor_probe.argtypes = [p, p, p, p, i64, i64, i64, p]
     lib.swiglu_launch_floor_probe.restype = ci
     lib.swiglu_last_error.argtypes, lib.swiglu_last_error.restype = [], ctypes.c_char_p
@@ -334,6 +339,18 @@ def swiglu_glu_mlp_packed(A, Wp, Y, activation="silu", variant=-1, M=None, N=Non
         N = int(Y.shape[1])
     _check(load().swiglu_glu_mlp_packed(_ptr(A), _ptr(Wp), _ptr(Y), int(M), int(N), int(K),
                                         _act(activation), int(variant), _stream(stream)))
+
+
+def swiglu_mlp_fp8(A8, W1_8, W2_8, Y, scale_gate=1.0, scale_up=1.0, variant=-1, M=None, N=None,
+                   K=None, stream=None) -> None:
+    """FP8 (E4M3) operands: Y = bf16(SiLU(scale_gate * A8.W1_8^T) * (scale_up * A8.W2_8^T));
+    A8 [M,K], W1_8 / W2_8 [N,K] one byte per element, Y [M,N] bf16."""
+    if M is None:
+        M, K = int(A8.shape[0]), int(A8.shape[1])
+        N = int(Y.shape[1])
+    _check(load().swiglu_mlp_fp8_ex(_ptr(A8), _ptr(W1_8), _ptr(W2_8), _ptr(Y), int(M), int(N),
+                                    int(K), float(scale_gate), float(scale_up), int(variant),
+                                    _stream(stream)))
 
 
 def swiglu_launch_floor_probe(A, W1, W2, Y, M=None, N=None, K=None, stream=None) -> None:

@@ -63,6 +63,7 @@ struct GemmParams {
   int early_issue;      // 1: fill the ring before the CTA-wide setup barrier (small grids)
   int w_evict_first;    // 1: weights are read once (one row of tiles): L2 evict-first loads
   unsigned long long* clk;  // optional {SM cycles, globaltimer ns} of CTA 0 (swiglu_set_clock_probe)
+  float scale_gate, scale_up;  // kOperandsFp8: Gate / Up dequantisation scales (else unused)
 #ifdef SWIGLU_TRACE
   unsigned long long* trace;  // [grid][kGemmTraceStride] globaltimer stamps (debug builds only)
 #endif
@@ -203,7 +204,12 @@ __device__ __forceinline__ float glu_mul(float g, float u) {
 //     [n-tile][g0,u0,g1,u1][K][64], so ONE 3-D TMA box per stage fetches Gate|Up slabs
 //     (tmap_b1: the multi-slab box; tmap_b2: a single-slab box for 2-CTA / 1-CTA half tiles).
 //     MN-major like KN; accumulator columns come out as g0 u0 g1 u1.
-enum : int { kWeightsKN = 0, kWeightsNK = 1, kWeightsPacked = 2 };
+//   kOperandsFp8: A [M,K] AND both weight matrices [N,K] are OCP FP8 E4M3 bytes (PAPER.md lines
+//     382, 392 item 2): K-major operands, a k-block is 128 elements (the
+//     same 128-byte rows, so every shared-memory size and descriptor stride is unchanged),
+//     tcgen05.mma kind::f8f6f4 with 32 k per instruction, and the per-projection dequantisation
+//     scales multiply the fp32 accumulators in the epilogue before the activation.
+enum : int { kWeightsKN = 0, kWeightsNK = 1, kWeightsPacked = 2, kOperandsFp8 = 3 };
 
 template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = kActSilu, int kWMode = kWeightsKN>
 __global__ void __launch_bounds__(kGemmThreads, 1)
@@ -213,8 +219,11 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                    const __grid_constant__ CUtensorMap tmap_y, const GemmParams p) {
   static_assert(kBN == 128 || (kBN == 64 && kFused && kCtaGroup == 1), "narrow tile: fused 1-CTA");
   static_assert(kWMode != kWeightsPacked || kFused, "packed weights: fused path only");
-  constexpr bool kWK = (kWMode == kWeightsNK);
+  static_assert(kWMode != kOperandsFp8 || kFused, "FP8 operands: fused path only");
+  constexpr bool kF8 = (kWMode == kOperandsFp8);
+  constexpr bool kWK = (kWMode == kWeightsNK) || kF8;
   constexpr bool kPacked = (kWMode == kWeightsPacked);
+  constexpr int kBKe = kF8 ? 128 : BK;            // elements of k per stage (128-byte rows)
   constexpr int UMMA_N = kFused ? 2 * kBN : 256;  // accumulator columns per tile
   using Cfg = GemmCfg<kCtaGroup, UMMA_N>;
   constexpr int kStages = Cfg::kStages;
@@ -240,7 +249,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   const int num_groups = gridDim.x / kCtaGroup;  // CTAs (or CTA pairs) sharing the tile list
   const int group_id = blockIdx.x / kCtaGroup;
   const int total_tiles = p.total_tiles;
-  const int k_blocks = (p.K + BK - 1) / BK;
+  const int k_blocks = (p.K + kBKe - 1) / kBKe;
 
   // A single row of tiles reads every weight byte exactly once: stream it past L2 (evict-first).
   const uint64_t w_policy = p.w_evict_first ? kEvictFirst : kEvictNormal;
@@ -252,7 +261,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       const uint32_t b_bytes = half ? Cfg::kBBytes / 2 : Cfg::kBBytes;
       mbar_arrive_expect_tx(full_bar(s), (Cfg::kABytes + b_bytes) * kCtaGroup);
     }
-    const int k0 = kb * BK;
+    const int k0 = kb * kBKe;
     const uint32_t sa = smem_a(s), sb = smem_b(s), fb = full_bar(s);
     // one 64-column x 64-k weight slab; the tensor map's inner dimension is N ([K,N]) or K ([N,K])
     auto load_w = [&](uint32_t dst, const CUtensorMap* tm, int n) {
@@ -371,9 +380,11 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     }
   } else if (warp == 1 && lane == 0 && rank == 0) {
     // ================================================================ MMA issuer
-    constexpr uint32_t idesc_full = idesc_bf16_f32(BM * kCtaGroup, UMMA_N, /*a_mn=*/false,
-                                                   /*b_mn=*/!kWK);
-    constexpr uint32_t idesc_half = idesc_bf16_f32(BM * kCtaGroup, 128, false, !kWK);
+    constexpr uint32_t idesc_full =
+        kF8 ? idesc_e4m3_f32(BM * kCtaGroup, UMMA_N)
+            : idesc_bf16_f32(BM * kCtaGroup, UMMA_N, /*a_mn=*/false, /*b_mn=*/!kWK);
+    constexpr uint32_t idesc_half = kF8 ? idesc_e4m3_f32(BM * kCtaGroup, 128)
+                                        : idesc_bf16_f32(BM * kCtaGroup, 128, false, !kWK);
     int s = 0;
     uint32_t ph = 0;
     int it = 0;
@@ -400,7 +411,8 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           // B, [N,K] weights: K-major like A (slabs of 64 n-rows are 8 KB = 8 groups of 8 rows).
           const uint64_t bdesc = kWK ? smem_desc_sw128(sb + k * (UMMA_K * 2), 16, 1024)
                                      : smem_desc_sw128(sb + k * (UMMA_K * 128), 8192, 1024);
-          umma_bf16<kCtaGroup>(d_tmem, adesc, bdesc, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
+          if constexpr (kF8) umma_f8<kCtaGroup>(d_tmem, adesc, bdesc, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
+          else umma_bf16<kCtaGroup>(d_tmem, adesc, bdesc, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
         }
         umma_commit<kCtaGroup>(empty_bar(s));  // smem stage free once these MMAs retire
         if (++s == kStages) { s = 0; ph ^= 1u; }
@@ -513,11 +525,13 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
             }
 #pragma unroll
             for (int j = 0; j < 16; ++j) {
-              const float y0 =
-                  glu_mul<kAct>(__uint_as_float(g[2 * j]), __uint_as_float(u[2 * j]));
-              const float y1 =
-                  glu_mul<kAct>(__uint_as_float(g[2 * j + 1]), __uint_as_float(u[2 * j + 1]));
-              packed[j] = pack_bf16x2_rn(y0, y1);
+              float g0 = __uint_as_float(g[2 * j]), u0 = __uint_as_float(u[2 * j]);
+              float g1 = __uint_as_float(g[2 * j + 1]), u1 = __uint_as_float(u[2 * j + 1]);
+              if constexpr (kF8) {  // dequantise: one scale per projection
+                g0 *= p.scale_gate; g1 *= p.scale_gate;
+                u0 *= p.scale_up; u1 *= p.scale_up;
+              }
+              packed[j] = pack_bf16x2_rn(glu_mul<kAct>(g0, u0), glu_mul<kAct>(g1, u1));
             }
           } else {
             uint32_t v[32];

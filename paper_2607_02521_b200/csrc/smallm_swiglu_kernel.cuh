@@ -57,6 +57,7 @@ struct SmallParams {
   long long ldy;      // = N
   uint16_t* U;        // kStoreGU only: bf16 Up output (Gate goes to the Y argument)
   unsigned long long* clk;  // optional {SM cycles, globaltimer ns} of CTA 0 (swiglu_set_clock_probe)
+  float scale_gate, scale_up;  // kOperandsFp8: Gate / Up dequantisation scales (else unused)
 #ifdef SWIGLU_TRACE
   unsigned long long* trace;  // [grid][16] globaltimer stamps (debug builds only)
 #endif
@@ -83,8 +84,10 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                      const SmallParams p) {
   using Cfg = SmallCfg<MP>;
   constexpr int kStages = Cfg::kStages;
-  constexpr bool kWK = (kWMode == kWeightsNK);
+  constexpr bool kF8 = (kWMode == kOperandsFp8);   // E4M3 A and [N,K] weights (gemm kernel header)
+  constexpr bool kWK = (kWMode == kWeightsNK) || kF8;
   constexpr bool kPacked = (kWMode == kWeightsPacked);
+  constexpr int kBKe = kF8 ? 128 : BK;              // elements of k per stage (128-byte rows)
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bar_base = smem_base + kStages * Cfg::kStageBytes;
@@ -102,7 +105,7 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   const uint32_t rank = (S > 1) ? cluster_ctarank() : 0u;
   const int n_tile = blockIdx.x / S;
   const int n_base = n_tile * 128;
-  const int k_blocks = (p.K + BK - 1) / BK;
+  const int k_blocks = (p.K + kBKe - 1) / kBKe;
   const int kb_begin = (int)(((long long)k_blocks * rank) / S);
   const int kb_end = (int)(((long long)k_blocks * (rank + 1)) / S);
 
@@ -110,7 +113,7 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   // call: evict-first, so they do not push A out of L2.
   auto issue_w = [&](int kb, int s) {
     const uint32_t fb = full_bar(s);
-    const int k0 = kb * BK;
+    const int k0 = kb * kBKe;
     if constexpr (kPacked) {
       tma_load_3d(smem_w(s), &tmap_w1, fb, 0, k0, n_tile * 4, kEvictFirst);  // g0 u0 g1 u1: 32 KB
     } else {
@@ -125,7 +128,7 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     }
   };
   auto issue_a = [&](int kb, int s) {
-    tma_load_2d(smem_act(s), &tmap_a, full_bar(s), kb * BK, 0, kEvictLast);
+    tma_load_2d(smem_act(s), &tmap_a, full_bar(s), kb * kBKe, 0, kEvictLast);
   };
 
   if (threadIdx.x == 0) SWIGLU_TRACE_POINT(0);
@@ -160,7 +163,7 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       // the rest of the CTA's weight stream: L2 prefetch, one k-block per lane
       const int kb = kb_begin + kStages + (int)lane;
       if (live && (int)lane < p.prefetch_blocks && kb < kb_end)
-        tma_prefetch_l2_3d(&tmap_w1, 0, kb * BK, n_tile * 4);
+        tma_prefetch_l2_3d(&tmap_w1, 0, kb * kBKe, n_tile * 4);
       if (lane == 0 && live) {
         pdl_wait_prior_grid();  // A may be the previous kernel's output
         SWIGLU_TRACE_POINT(2);
@@ -170,7 +173,7 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       // L2 prefetch of this CTA's weight stream (hint; legal before griddepcontrol.wait)
       const int kb = kb_begin + (int)lane;
       if (live && (int)lane < p.prefetch_blocks && kb < kb_end) {
-        const int k0 = kb * BK;
+        const int k0 = kb * kBKe;
         tma_prefetch_l2_2d(&tmap_w1, kWK ? k0 : n_base, kWK ? n_base : k0);
         tma_prefetch_l2_2d(&tmap_w1, kWK ? k0 : n_base + 64, kWK ? n_base + 64 : k0);
         tma_prefetch_l2_2d(&tmap_w2, kWK ? k0 : n_base, kWK ? n_base : k0);
@@ -212,7 +215,8 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       }
     } else if (warp == 1 && lane == 0) {
       // ================================================================ MMA issuer
-      constexpr uint32_t idesc = idesc_bf16_f32(128, MP, /*a_mn=*/!kWK, /*b_mn=*/false);
+      constexpr uint32_t idesc = kF8 ? idesc_e4m3_f32(128, MP)
+                                     : idesc_bf16_f32(128, MP, /*a_mn=*/!kWK, /*b_mn=*/false);
       int s = 0;
       uint32_t ph = 0;
       for (int kb = kb_begin; kb < kb_end; ++kb) {
@@ -240,8 +244,13 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           }
           // activations: K-major "B" operand, +32 B per step inside the swizzle row
           const uint64_t ad = smem_desc_sw128(smem_act(s) + k * (UMMA_K * 2), 16, 1024);
-          umma_bf16<1>(tmem_base, w1d, ad, idesc, acc);       // Gate^T -> columns [0, MP)
-          umma_bf16<1>(tmem_base + MP, w2d, ad, idesc, acc);  // Up^T   -> columns [MP, 2MP)
+          if constexpr (kF8) {
+            umma_f8<1>(tmem_base, w1d, ad, idesc, acc);
+            umma_f8<1>(tmem_base + MP, w2d, ad, idesc, acc);
+          } else {
+            umma_bf16<1>(tmem_base, w1d, ad, idesc, acc);       // Gate^T -> columns [0, MP)
+            umma_bf16<1>(tmem_base + MP, w2d, ad, idesc, acc);  // Up^T   -> columns [MP, 2MP)
+          }
         }
         umma_commit<1>(empty_bar(s));
         if (++s == kStages) { s = 0; ph ^= 1u; }
@@ -305,7 +314,11 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       uint32_t peer[8];
 #pragma unroll
       for (int r = 0; r < 8; ++r) peer[r] = (r < S) ? mapa_shared(part, (uint32_t)r) : 0u;
-      auto finish_row = [&](int m, const float4& gs, const float4& us) {
+      auto finish_row = [&](int m, float4 gs, float4 us) {
+        if constexpr (kF8) {  // dequantise: one scale per projection
+          gs.x *= p.scale_gate; gs.y *= p.scale_gate; gs.z *= p.scale_gate; gs.w *= p.scale_gate;
+          us.x *= p.scale_up; us.y *= p.scale_up; us.z *= p.scale_up; us.w *= p.scale_up;
+        }
         if (n < p.N) {  // N % 8 == 0 and n % 4 == 0: the 4 columns are in range together
           if constexpr (kStoreGU) {
             *reinterpret_cast<uint2*>(Y + (long long)m * p.ldy + n) =

@@ -21,6 +21,7 @@ namespace {
 using swiglu::kWeightsKN;
 using swiglu::kWeightsNK;
 using swiglu::kWeightsPacked;
+using swiglu::kOperandsFp8;
 
 // ------------------------------------------------------------------ error bookkeeping
 thread_local char g_err[512] = "";
@@ -211,7 +212,7 @@ int set_smem_attrs() {
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kAct, kWK>, attr, SmallCfg<32>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kAct, kWK>, attr, SmallCfg<64>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<128, kAct, kWK>, attr, SmallCfg<128>::kSmemBytes));
-  if constexpr (kAct == kActSilu && kWK != kWeightsPacked) {  // the unfused path's plain GEMMs have no activation
+  if constexpr (kAct == kActSilu && kWK != kWeightsPacked && kWK != kOperandsFp8) {  // plain GEMMs: no activation
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kActSilu, kWK, true>, attr, SmallCfg<16>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kActSilu, kWK, true>, attr, SmallCfg<32>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kActSilu, kWK, true>, attr, SmallCfg<64>::kSmemBytes));
@@ -252,7 +253,8 @@ int get_device_state(DeviceState** out) {
         (rc = set_smem_attrs<kActSilu, kWeightsNK>()) || (rc = set_smem_attrs<kActGelu, kWeightsNK>()) ||
         (rc = set_smem_attrs<kActGeluTanh, kWeightsNK>()) || (rc = set_smem_attrs<kActRelu, kWeightsNK>()) ||
         (rc = set_smem_attrs<kActSilu, kWeightsPacked>()) || (rc = set_smem_attrs<kActGelu, kWeightsPacked>()) ||
-        (rc = set_smem_attrs<kActGeluTanh, kWeightsPacked>()) || (rc = set_smem_attrs<kActRelu, kWeightsPacked>()))
+        (rc = set_smem_attrs<kActGeluTanh, kWeightsPacked>()) || (rc = set_smem_attrs<kActRelu, kWeightsPacked>()) ||
+        (rc = set_smem_attrs<kActSilu, kOperandsFp8>()))
       return rc;
     d.ready = true;
   }
@@ -264,10 +266,10 @@ int get_device_state(DeviceState** out) {
 // (base, dims, box): a cached copy can never be stale, whatever happened to the
 // allocation in between.  Thread-local and direct-mapped, so the hot path takes no lock.
 struct TmapKey {
-  const void* base; int64_t d0, d1, d2; uint32_t b0, b1, b2;
+  const void* base; int64_t d0, d1, d2; uint32_t b0, b1, b2; uint32_t esize;  // 2 = bf16, 1 = fp8
   bool operator==(const TmapKey& o) const {
     return base == o.base && d0 == o.d0 && d1 == o.d1 && d2 == o.d2 && b0 == o.b0 && b1 == o.b1 &&
-           b2 == o.b2;
+           b2 == o.b2 && esize == o.esize;
   }
 };
 struct TmapSlot { bool used = false; TmapKey key; CUtensorMap map; };
@@ -275,16 +277,18 @@ constexpr int kTmapSlots = 256;
 thread_local TmapSlot t_tmaps[kTmapSlots];
 thread_local uint64_t t_tmap_hits = 0, t_tmap_misses = 0;
 
-// bf16 tensor, dense row-major, dims innermost first (d2 == 0: 2-D), box b0 x b1 [x b2],
-// 128-byte swizzle (b0 must be 64 elements), out-of-bounds reads give zeros.
+// bf16 (or 1-byte) tensor, dense row-major, dims innermost first (d2 == 0: 2-D), box b0 x b1
+// [x b2], 128-byte swizzle (b0 * esize must be 128 bytes), out-of-bounds reads give zeros.
 int encode_tmap(CUtensorMap* out, const TmapKey& k) {
   const cuuint32_t rank = k.d2 ? 3 : 2;
   const cuuint64_t dims[3] = {(cuuint64_t)k.d0, (cuuint64_t)k.d1, (cuuint64_t)k.d2};
-  const cuuint64_t strides[2] = {(cuuint64_t)k.d0 * 2, (cuuint64_t)k.d0 * 2 * (cuuint64_t)k.d1};
+  const cuuint64_t strides[2] = {(cuuint64_t)k.d0 * k.esize,
+                                 (cuuint64_t)k.d0 * k.esize * (cuuint64_t)k.d1};
   const cuuint32_t box[3] = {k.b0, k.b1, k.b2};
   const cuuint32_t elem[3] = {1, 1, 1};
   const CUresult r =
-      g_encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, rank, const_cast<void*>(k.base), dims,
+      g_encode(out, k.esize == 1 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16,
+               rank, const_cast<void*>(k.base), dims,
                strides, box, elem, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS)
@@ -297,7 +301,8 @@ int cached_tmap(CUtensorMap* out, const TmapKey& key) {
   if (env().no_tmap_cache) return encode_tmap(out, key);
   uint64_t h = (uint64_t)(uintptr_t)key.base * 0x9E3779B97F4A7C15ull;
   h ^= ((uint64_t)key.d0 * 0xC2B2AE3D27D4EB4Full) ^ ((uint64_t)key.d1 * 0x165667B19E3779F9ull) ^
-       ((uint64_t)key.d2 * 0x27D4EB2F165667C5ull) ^ ((uint64_t)key.b1 << 7) ^ ((uint64_t)key.b2 << 17);
+       ((uint64_t)key.d2 * 0x27D4EB2F165667C5ull) ^ ((uint64_t)key.b1 << 7) ^ ((uint64_t)key.b2 << 17) ^
+       ((uint64_t)key.esize << 27);
   TmapSlot& slot = t_tmaps[(h >> 40) & (kTmapSlots - 1)];
   if (slot.used && slot.key == key) {
     ++t_tmap_hits;
@@ -316,12 +321,17 @@ int cached_tmap(CUtensorMap* out, const TmapKey& key) {
 // 2-D tensor [outer, inner] (inner contiguous), box = box_outer x box_inner.
 int make_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
               uint32_t box_inner, uint32_t box_outer) {
-  return cached_tmap(out, TmapKey{base, inner, outer, 0, box_inner, box_outer, 0});
+  return cached_tmap(out, TmapKey{base, inner, outer, 0, box_inner, box_outer, 0, 2});
+}
+// FP8 (1-byte) 2-D tensor [outer, inner]: a box row is 128 elements = 128 bytes.
+int make_tmap_u8(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
+                 uint32_t box_outer) {
+  return cached_tmap(out, TmapKey{base, inner, outer, 0, 128, box_outer, 0, 1});
 }
 // Prepacked weights Wp[slab][k][64]: {64, K, slabs}, box = 64 x 64 x box_slabs.
 int make_tmap_packed(CUtensorMap* out, const void* base, int64_t K, int64_t slabs,
                      uint32_t box_slabs) {
-  return cached_tmap(out, TmapKey{base, 64, K, slabs, 64, 64, box_slabs});
+  return cached_tmap(out, TmapKey{base, 64, K, slabs, 64, 64, box_slabs, 2});
 }
 inline int64_t packed_slabs(int64_t N) { return 4 * ((N + 127) / 128); }
 
@@ -365,13 +375,22 @@ TailPlan plan_tail(int64_t tiles, int G, int64_t k_blocks, bool fused128, bool h
 // ------------------------------------------------------------------ launches
 template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = swiglu::kActSilu, int kWMode = 0>
 int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void* B2, void* Yout,
-                int64_t M, int64_t N, int64_t K, cudaStream_t stream, void* split_ws = nullptr) {
+                int64_t M, int64_t N, int64_t K, cudaStream_t stream, void* split_ws = nullptr,
+                float scale_gate = 1.0f, float scale_up = 1.0f) {
   using namespace swiglu;
   CUtensorMap ta, tb1, tb2, ty;
   int rc;
   constexpr bool kWK = (kWMode == kWeightsNK);
-  if ((rc = make_tmap(&ta, A, K, M, 64, 128))) return rc;
-  if constexpr (kWMode == kWeightsPacked) {
+  constexpr int kBKe = (kWMode == kOperandsFp8) ? 128 : BK;   // k elements per stage
+  if constexpr (kWMode == kOperandsFp8) {
+    if ((rc = make_tmap_u8(&ta, A, K, M, 128))) return rc;
+    if ((rc = make_tmap_u8(&tb1, B1, K, N, 64))) return rc;    // [N,K] E4M3: 64 n-rows x 128 k
+    if ((rc = make_tmap_u8(&tb2, B2, K, N, 64))) return rc;
+  } else if ((rc = make_tmap(&ta, A, K, M, 64, 128))) {
+    return rc;
+  }
+  if constexpr (kWMode == kOperandsFp8) {
+  } else if constexpr (kWMode == kWeightsPacked) {
     // B1 = Wp: one box per stage -- 4 slabs (1-CTA, 128 columns) or 2 (64-column tile; each
     // CTA of a pair); single-slab boxes for the half tiles of the last wave
     const uint32_t box = (kCtaGroup == 1 && kBN == 128) ? 4 : 2;
@@ -391,7 +410,7 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   p.m_tiles = (int)((M + rows_per_tile - 1) / rows_per_tile);
   p.n_tiles = (int)((N + out_cols - 1) / out_cols);
   // L2 raster group: keep the slab of A the running CTAs share at <= 32 MiB
-  int64_t gm = (32ll << 20) / ((int64_t)rows_per_tile * K * 2);
+  int64_t gm = (32ll << 20) / ((int64_t)rows_per_tile * K * (kWMode == kOperandsFp8 ? 1 : 2));
   const int forced_gm = env().group_m;
   if (forced_gm > 0) gm = forced_gm;
   if (gm < 1) gm = 1;
@@ -399,7 +418,7 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   p.group_m = (int)gm;
   const int64_t tiles = (int64_t)p.m_tiles * p.n_tiles;
   const int G = d.sm_count / kCtaGroup;
-  const TailPlan tail = plan_tail(tiles, G, (K + BK - 1) / BK, kFused && kBN == 128,
+  const TailPlan tail = plan_tail(tiles, G, (K + kBKe - 1) / kBKe, kFused && kBN == 128,
                                   split_ws != nullptr && d.sm_count <= 160);
   p.wide_tiles = (int)tail.wide;
   p.total_tiles = (int)tail.total;
@@ -411,6 +430,8 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   p.early_issue = (kCtaGroup == 1 && kFused && tiles <= groups && tail.ksplit == 0 && !env().no_early);
   p.w_evict_first = (p.m_tiles == 1 && !env().no_w_evict_first);
   p.clk = g_clk.load(std::memory_order_relaxed);
+  p.scale_gate = scale_gate;
+  p.scale_up = scale_up;
 #ifdef SWIGLU_TRACE
   p.trace = g_trace;
 #endif
@@ -470,26 +491,36 @@ int smallm_ksplit(int sm_count, int ctas_per_sm, int mp, int64_t n_tiles, int64_
 template <int MP, int kAct, int kWMode, bool kStoreGU = false>
 int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const void* W2,
                      void* Y, void* U, int64_t M, int64_t N, int64_t K, cudaStream_t stream,
-                     int probe = 0) {
+                     int probe = 0, float scale_gate = 1.0f, float scale_up = 1.0f) {
   using namespace swiglu;
   constexpr bool kWK = (kWMode == kWeightsNK);
+  constexpr int kBKe = (kWMode == kOperandsFp8) ? 128 : BK;
   CUtensorMap ta, tw1, tw2;
   int rc;
-  if ((rc = make_tmap(&ta, A, K, M, 64, MP))) return rc;
-  if constexpr (kWMode == kWeightsPacked) {
+  if constexpr (kWMode == kOperandsFp8) {
+    if ((rc = make_tmap_u8(&ta, A, K, M, MP))) return rc;
+    if ((rc = make_tmap_u8(&tw1, W1, K, N, 64))) return rc;
+    if ((rc = make_tmap_u8(&tw2, W2, K, N, 64))) return rc;
+  } else if ((rc = make_tmap(&ta, A, K, M, 64, MP))) {
+    return rc;
+  }
+  if constexpr (kWMode == kOperandsFp8) {
+  } else if constexpr (kWMode == kWeightsPacked) {
     if ((rc = make_tmap_packed(&tw1, W1, K, packed_slabs(N), 4))) return rc;  // W1 = Wp
     tw2 = tw1;
   } else {
     if ((rc = make_tmap(&tw1, W1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
     if ((rc = make_tmap(&tw2, W2, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
   }
-  const int64_t n_tiles = (N + 127) / 128, k_blocks = (K + BK - 1) / BK;
+  const int64_t n_tiles = (N + 127) / 128, k_blocks = (K + kBKe - 1) / kBKe;
   SmallParams p;
   p.M = (int)M; p.N = (int)N; p.K = (int)K;
   p.ksplit = smallm_ksplit(d.sm_count, SmallCfg<MP>::kCtasPerSm, MP, n_tiles, k_blocks);
   p.ldy = N;
   p.U = (uint16_t*)U;
   p.probe = probe;
+  p.scale_gate = scale_gate;
+  p.scale_up = scale_up;
   p.clk = g_clk.load(std::memory_order_relaxed);
   // L2 prefetch ahead of the grid dependency: at most ~32 MiB over the whole grid
   const int64_t grid = n_tiles * p.ksplit;
@@ -529,11 +560,12 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
 
 template <int kAct, int kWMode, bool kStoreGU = false>
 int launch_smallm(const DeviceState& d, const void* A, const void* W1, const void* W2, void* Y,
-                  void* U, int64_t M, int64_t N, int64_t K, cudaStream_t stream, int probe = 0) {
-  if (M <= 16) return launch_smallm_mp<16, kAct, kWMode, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream, probe);
-  if (M <= 32) return launch_smallm_mp<32, kAct, kWMode, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream, probe);
-  if (M <= 64) return launch_smallm_mp<64, kAct, kWMode, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream, probe);
-  return launch_smallm_mp<128, kAct, kWMode, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream, probe);
+                  void* U, int64_t M, int64_t N, int64_t K, cudaStream_t stream, int probe = 0,
+                  float sg = 1.0f, float su = 1.0f) {
+  if (M <= 16) return launch_smallm_mp<16, kAct, kWMode, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream, probe, sg, su);
+  if (M <= 32) return launch_smallm_mp<32, kAct, kWMode, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream, probe, sg, su);
+  if (M <= 64) return launch_smallm_mp<64, kAct, kWMode, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream, probe, sg, su);
+  return launch_smallm_mp<128, kAct, kWMode, kStoreGU>(d, A, W1, W2, Y, U, M, N, K, stream, probe, sg, su);
 }
 
 template <int kAct>
@@ -874,6 +906,64 @@ int swiglu_glu_mlp_packed(const void* A, const void* Wp, void* Y, int64_t M, int
                           int activation, int variant, void* stream) {
   return run_fused(A, Wp, Wp, Y, M, N, K, variant, activation, swiglu::kWeightsPacked,
                    (cudaStream_t)stream);
+}
+
+// FP8 (E4M3) operands; see include/swiglu_mlp.h.
+static int run_fp8(const void* A8, const void* W1, const void* W2, void* Y, int64_t M, int64_t N,
+                   int64_t K, float sg, float su, int variant, cudaStream_t stream) {
+  if (M < 0 || N <= 0 || K <= 0)
+    return fail(SWIGLU_ERR_BAD_SHAPE, "bad shape M=%lld N=%lld K=%lld (need M>=0, N>0, K>0)",
+                (long long)M, (long long)N, (long long)K);
+  if (M > INT32_MAX - 256 || N > INT32_MAX - 256 || K > INT32_MAX - 256 ||
+      mul_overflows(M, K, INT64_MAX / 4) || mul_overflows(K, N, INT64_MAX / 4) ||
+      mul_overflows(M, N, INT64_MAX / 4))
+    return fail(SWIGLU_ERR_BAD_SHAPE, "shape too large M=%lld N=%lld K=%lld", (long long)M,
+                (long long)N, (long long)K);
+  if ((K % 16) != 0 || (N % 8) != 0)
+    return fail(SWIGLU_ERR_UNSUPPORTED,
+                "FP8: K=%lld must be a multiple of 16 and N=%lld of 8 (16-byte row pitch for TMA)",
+                (long long)K, (long long)N);
+  if (!(sg == sg) || !(su == su)) return fail(SWIGLU_ERR_UNSUPPORTED, "a scale is NaN");
+  if (variant < -1 || variant >= kNumFused)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
+  if (variant == kFusedSmallM && M > swiglu::kSmallMMax)
+    return fail(SWIGLU_ERR_UNSUPPORTED, "variant %s handles M <= %d only",
+                kFusedNames[kFusedSmallM], swiglu::kSmallMMax);
+  if (M == 0) return SWIGLU_OK;
+  if (!A8 || !W1 || !W2 || !Y) return fail(SWIGLU_ERR_NULL_POINTER, "A, W1, W2 or Y is NULL");
+  if (((uintptr_t)A8 | (uintptr_t)W1 | (uintptr_t)W2 | (uintptr_t)Y) & 15u)
+    return fail(SWIGLU_ERR_MISALIGNED, "A, W1, W2 and Y must be 16-byte aligned");
+  if (overlaps(Y, M * N * 2, A8, M * K) || overlaps(Y, M * N * 2, W1, K * N) ||
+      overlaps(Y, M * N * 2, W2, K * N))
+    return fail(SWIGLU_ERR_ALIASING, "Y overlaps an input");
+  DeviceState* d;
+  int rc;
+  if ((rc = get_device_state(&d))) return rc;
+  if (variant < 0) variant = select_fused(M, N, K);
+  using namespace swiglu;
+  void* split_ws = workspace_for(M, N, K / 2, 0, variant) > 0 ? split_workspace(*d, stream) : nullptr;
+  switch (variant) {
+    case kFused1Cta:
+      return launch_gemm<1, true, 128, kActSilu, kOperandsFp8>(*d, A8, W1, W2, Y, M, N, K, stream, split_ws, sg, su);
+    case kFused2Cta:
+      return launch_gemm<2, true, 128, kActSilu, kOperandsFp8>(*d, A8, W1, W2, Y, M, N, K, stream, split_ws, sg, su);
+    case kFusedSmallM:
+      return launch_smallm<kActSilu, kOperandsFp8>(*d, A8, W1, W2, Y, nullptr, M, N, K, stream, 0, sg, su);
+    case kFused1CtaN64:
+      return launch_gemm<1, true, 64, kActSilu, kOperandsFp8>(*d, A8, W1, W2, Y, M, N, K, stream, nullptr, sg, su);
+  }
+  return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
+}
+
+int swiglu_mlp_fp8(const void* A8, const void* W1_8, const void* W2_8, void* Y, int64_t M,
+                   int64_t N, int64_t K, float scale_gate, float scale_up, void* stream) {
+  return run_fp8(A8, W1_8, W2_8, Y, M, N, K, scale_gate, scale_up, -1, (cudaStream_t)stream);
+}
+
+int swiglu_mlp_fp8_ex(const void* A8, const void* W1_8, const void* W2_8, void* Y, int64_t M,
+                      int64_t N, int64_t K, float scale_gate, float scale_up, int variant,
+                      void* stream) {
+  return run_fp8(A8, W1_8, W2_8, Y, M, N, K, scale_gate, scale_up, variant, (cudaStream_t)stream);
 }
 
 int swiglu_launch_floor_probe(const void* A, const void* W1, const void* W2, void* Y, int64_t M,

@@ -20,7 +20,7 @@ def lib():
 def test_every_declared_symbol_is_exported(lib):
     header = open(os.path.join(ROOT, "include", "swiglu_mlp.h")).read()
     header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
-    declared = set(re.findall(r"\b(swiglu_[a-z_]+)\s*\(", header))
+    declared = set(re.findall(r"\b(swiglu_[a-z0-9_]+)\s*\(", header))
     assert declared == set(B.EXPORTS)
     for name in declared:
         assert hasattr(lib, name), name
