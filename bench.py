@@ -867,6 +867,50 @@ def run_fp8(args):
     print(json.dumps({"peak_source": peak_src, "fp8_peak_tflops": 2 * peaks["bf16_tflops"]}))
 
 
+def run_ncu_points(args):
+    """`--ncu-points name:M[:u][,name:M...]`: the kernels behind the per-point claims, launched
+    eagerly so that `ncu -k regex:... --set full` can capture them one by one: per point one
+    warm-up call and one more of swiglu_mlp (":u" adds swiglu_mlp_unfused, ":p" the prepacked
+    form, ":8" the FP8 form).  Weight copies rotate as in the timed runs (cold L2).  Prints one
+    line per point with the CUDA-event time of the last call -- NOT a bench value when run
+    under a profiler."""
+    import torch
+    from paper_2607_02521_b200 import binding as B, inputs
+    lib = B.load()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    cache = {}
+    for spec in args.ncu_points.split(","):
+        parts = spec.split(":")
+        name, M, flags = parts[0], int(parts[1]), "".join(parts[2:])
+        if name not in cache:
+            cache.clear()
+            torch.cuda.empty_cache()
+            cache[name] = Workload(name, Ms=[M])
+        wl = cache[name]
+        fns = [("fused", lib.swiglu_mlp)]
+        if "u" in flags:
+            fns.append(("unfused", lib.swiglu_mlp_unfused))
+        if "p" in flags:
+            nbytes = B.swiglu_packed_weight_bytes(wl.N, wl.K)
+            Wp = torch.empty(nbytes // 2, dtype=torch.int16, device="cuda")
+            B.swiglu_pack_weights(wl.W1[0], wl.W2[0], Wp, wl.N, wl.K)
+            fns.append(("packed", lambda a, w1, w2, y, m, n, k, st, _w=Wp: lib.swiglu_mlp_packed(
+                a, _w.data_ptr(), y, m, n, k, st)))
+        if "8" in flags:
+            A8h, W1h, W2h, sg, su = inputs.make_fp8_case(M, wl.N, wl.K, seed=50 + wl.seed)
+            A8, W18, W28 = (torch.from_numpy(x).cuda() for x in (A8h, W1h, W2h))
+            fns.append(("fp8", lambda a, w1, w2, y, m, n, k, st, _t=(A8, W18, W28, sg, su): lib.swiglu_mlp_fp8(
+                _t[0].data_ptr(), _t[1].data_ptr(), _t[2].data_ptr(), y, m, n, k, _t[3], _t[4], st)))
+        for label, fn in fns:
+            for i in range(2):
+                torch.cuda.synchronize()
+                e0.record()
+                wl.call(fn, M)
+                e1.record()
+                torch.cuda.synchronize()
+            print(f"{name} M={M} {label}: {e0.elapsed_time(e1) * 1e3:.1f} us (eager, second of 2 calls)", flush=True)
+
+
 def run_sweep(args):
     """Dispatch-table sweeps (`--sweep variants` / `--sweep ksplit`): time every fused variant
     (forced through swiglu_mlp_ex) or every split-K factor of the small-M kernel
@@ -952,6 +996,7 @@ def main():
     ap.add_argument("--sweep-batches", type=int, default=15)
     ap.add_argument("--decode-study", action="store_true")
     ap.add_argument("--fp8", action="store_true")
+    ap.add_argument("--ncu-points", default="")
     args = ap.parse_args()
     from paper_2607_02521_b200.dist import Ranks
     if args.impl == "reference":
@@ -973,6 +1018,9 @@ def main():
         return
     if args.fp8:
         run_fp8(args)
+        return
+    if args.ncu_points:
+        run_ncu_points(args)
         return
     ranks = Ranks()
     if ranks.world != args.gpus and ranks.rank == 0:

@@ -35,10 +35,14 @@ constexpr int kSmallMMax = 128;
 constexpr int kSmallThreads = 192;  // warp 0 TMA, warp 1 MMA, warps 2-5 epilogue
 constexpr int kSmallPrefetchMax = 32;     // k-blocks per CTA prefetched to L2 (one per lane)
 
-template <int MP>
+// kDeep: one CTA per SM with a six-stage ring (up to 204 KB of weights in flight per CTA) instead
+// of two co-resident CTAs with three stages each: half the CTAs (and clusters) to launch for the
+// same bytes in flight, used when n-tiles x S fits one CTA per SM (MP <= 32 only).
+template <int MP, bool kDeep = false>
 struct SmallCfg {
-  static constexpr int kCtasPerSm = (MP <= 64) ? 2 : 1;
-  static constexpr int kStages = (MP <= 32) ? 3 : (MP == 64 ? 2 : 4);
+  static_assert(!kDeep || MP <= 32, "deep ring: MP <= 32");
+  static constexpr int kCtasPerSm = kDeep ? 1 : ((MP <= 64) ? 2 : 1);
+  static constexpr int kStages = kDeep ? 6 : ((MP <= 32) ? 3 : (MP == 64 ? 2 : 4));
   static constexpr int kWBytes = 128 * BK * 2;  // one W tile: 128 n x 64 k = 16 KB
   static constexpr int kABytes = MP * BK * 2;   // MP tokens x 64 k
   static constexpr int kStageBytes = 2 * kWBytes + kABytes;
@@ -76,13 +80,14 @@ __device__ __forceinline__ float4 ld_dsmem_v4(uint32_t cluster_addr) {
 //   the reduced fp32 Gate and Up are each rounded to bf16 and written to HBM (Y argument = Gate,
 //   p.U = Up) instead of going through the activation -- one launch for both projections, the
 //   "merged gate_up_proj" serving stacks run before their silu_and_mul kernel.
-template <int MP, int kAct = kActSilu, int kWMode = kWeightsKN, bool kStoreGU = false>
-__global__ void __launch_bounds__(kSmallThreads, SmallCfg<MP>::kCtasPerSm)
+template <int MP, int kAct = kActSilu, int kWMode = kWeightsKN, bool kStoreGU = false,
+          bool kDeep = false>
+__global__ void __launch_bounds__(kSmallThreads, SmallCfg<MP, kDeep>::kCtasPerSm)
 smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                      const __grid_constant__ CUtensorMap tmap_w1,
                      const __grid_constant__ CUtensorMap tmap_w2, uint16_t* __restrict__ Y,
                      const SmallParams p) {
-  using Cfg = SmallCfg<MP>;
+  using Cfg = SmallCfg<MP, kDeep>;
   constexpr int kStages = Cfg::kStages;
   constexpr bool kF8 = (kWMode == kOperandsFp8);   // E4M3 A and [N,K] weights (gemm kernel header)
   constexpr bool kWK = (kWMode == kWeightsNK) || kF8;

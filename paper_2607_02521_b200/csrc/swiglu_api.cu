@@ -82,6 +82,7 @@ struct Env {
   int variant = -1, unfused_variant = -1, ksplit = 0, group_m = 0, host_chunks = 4, tail_ksplit = 0;
   bool no_pdl = false, no_prefetch = false, no_early = false, no_tail_split = false,
        no_tail_ksplit = false, no_w_evict_first = false, no_tmap_cache = false;
+  int smallm_deep = -1;  // -1 automatic, 0 never, 1 whenever it fits
 };
 Env g_env;
 std::once_flag g_env_once;
@@ -102,6 +103,7 @@ void load_env() {
   e.no_tail_ksplit = env_int("SWIGLU_NO_TAIL_KSPLIT", 0) != 0;
   e.no_w_evict_first = env_int("SWIGLU_NO_W_EVICT_FIRST", 0) != 0;
   e.no_tmap_cache = env_int("SWIGLU_NO_TMAP_CACHE", 0) != 0;
+  e.smallm_deep = env_int("SWIGLU_SMALLM_DEEP", -1);
   g_env = e;
 }
 const Env& env() {
@@ -212,6 +214,10 @@ int set_smem_attrs() {
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kAct, kWK>, attr, SmallCfg<32>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kAct, kWK>, attr, SmallCfg<64>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<128, kAct, kWK>, attr, SmallCfg<128>::kSmemBytes));
+  if constexpr (kWK == kWeightsKN || kWK == kWeightsPacked) {
+    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kAct, kWK, false, true>, attr, SmallCfg<16, true>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kAct, kWK, false, true>, attr, SmallCfg<32, true>::kSmemBytes));
+  }
   if constexpr (kAct == kActSilu && kWK != kWeightsPacked && kWK != kOperandsFp8) {  // plain GEMMs: no activation
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kActSilu, kWK, true>, attr, SmallCfg<16>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kActSilu, kWK, true>, attr, SmallCfg<32>::kSmemBytes));
@@ -488,11 +494,26 @@ int smallm_ksplit(int sm_count, int ctas_per_sm, int mp, int64_t n_tiles, int64_
   return (int)s;
 }
 
-template <int MP, int kAct, int kWMode, bool kStoreGU = false>
+template <int MP, int kAct, int kWMode, bool kStoreGU = false, bool kDeep = false>
 int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const void* W2,
                      void* Y, void* U, int64_t M, int64_t N, int64_t K, cudaStream_t stream,
                      int probe = 0, float scale_gate = 1.0f, float scale_up = 1.0f) {
   using namespace swiglu;
+  // Deep-ring form (one CTA per SM, six stages): taken when it is instantiated for this
+  // (MP, weights) and some S <= 4 puts n-tiles x S on at most one CTA per SM.
+  if constexpr (!kDeep && !kStoreGU && MP <= 32 && (kWMode == kWeightsKN || kWMode == kWeightsPacked)) {
+    const int64_t nt = (N + 127) / 128;
+    const bool fits = nt < d.sm_count && (env().ksplit <= 0 || nt * env().ksplit <= d.sm_count);
+    // automatic: only with prepacked (constant) weights and when the CTA's whole K-range fits the
+    // ring, so that every weight byte is in flight before griddepcontrol.wait (0.5B: 6.8 -> 6.1 us;
+    // with 12 k-blocks per CTA at 1.5B the two-CTA form stays ahead: profiles/r02_decode_study.md)
+    const int64_t s_deep = smallm_ksplit(d.sm_count, 1, MP, nt, (K + 63) / 64);
+    const bool resident = ((K + 63) / 64 + s_deep - 1) / s_deep <= SmallCfg<MP, true>::kStages;
+    const bool automatic = env().smallm_deep < 0 && kWMode == kWeightsPacked && resident;
+    if (fits && (env().smallm_deep == 1 || automatic))
+      return launch_smallm_mp<MP, kAct, kWMode, kStoreGU, true>(d, A, W1, W2, Y, U, M, N, K, stream,
+                                                                probe, scale_gate, scale_up);
+  }
   constexpr bool kWK = (kWMode == kWeightsNK);
   constexpr int kBKe = (kWMode == kOperandsFp8) ? 128 : BK;
   CUtensorMap ta, tw1, tw2;
@@ -515,7 +536,7 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   const int64_t n_tiles = (N + 127) / 128, k_blocks = (K + kBKe - 1) / kBKe;
   SmallParams p;
   p.M = (int)M; p.N = (int)N; p.K = (int)K;
-  p.ksplit = smallm_ksplit(d.sm_count, SmallCfg<MP>::kCtasPerSm, MP, n_tiles, k_blocks);
+  p.ksplit = smallm_ksplit(d.sm_count, SmallCfg<MP, kDeep>::kCtasPerSm, MP, n_tiles, k_blocks);
   p.ldy = N;
   p.U = (uint16_t*)U;
   p.probe = probe;
@@ -524,7 +545,7 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   p.clk = g_clk.load(std::memory_order_relaxed);
   // L2 prefetch ahead of the grid dependency: at most ~32 MiB over the whole grid
   const int64_t grid = n_tiles * p.ksplit;
-  int64_t pf = (32ll << 20) / (grid * 2 * SmallCfg<MP>::kWBytes);
+  int64_t pf = (32ll << 20) / (grid * 2 * SmallCfg<MP, kDeep>::kWBytes);
   if (pf > kSmallPrefetchMax) pf = kSmallPrefetchMax;
   if (env().no_prefetch) pf = 0;
   p.prefetch_blocks = (int)pf;
@@ -535,7 +556,7 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   memset(&cfg, 0, sizeof cfg);
   cfg.gridDim = dim3((unsigned)(n_tiles * p.ksplit));
   cfg.blockDim = dim3(kSmallThreads);
-  cfg.dynamicSmemBytes = SmallCfg<MP>::kSmemBytes;
+  cfg.dynamicSmemBytes = SmallCfg<MP, kDeep>::kSmemBytes;
   cfg.stream = stream;
   cudaLaunchAttribute attrs[2];
   int na = 0;
@@ -553,8 +574,8 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   }
   cfg.attrs = attrs;
   cfg.numAttrs = na;
-  CUDA_TRY(cudaLaunchKernelEx(&cfg, smallm_swiglu_kernel<MP, kAct, kWMode, kStoreGU>, ta, tw1, tw2,
-                              (uint16_t*)Y, p));
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, smallm_swiglu_kernel<MP, kAct, kWMode, kStoreGU, kDeep>, ta, tw1,
+                              tw2, (uint16_t*)Y, p));
   return SWIGLU_OK;
 }
 
