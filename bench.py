@@ -879,13 +879,13 @@ def run_ncu_points(args):
     lib = B.load()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     cache = {}
-    for spec in args.ncu_points.split(","):
-        parts = spec.split(":")
+    specs = [sp.split(":") for sp in args.ncu_points.split(",")]
+    for parts in specs:
         name, M, flags = parts[0], int(parts[1]), "".join(parts[2:])
         if name not in cache:
             cache.clear()
             torch.cuda.empty_cache()
-            cache[name] = Workload(name, Ms=[M])
+            cache[name] = Workload(name, Ms=[int(q[1]) for q in specs if q[0] == name])
         wl = cache[name]
         fns = [("fused", lib.swiglu_mlp)]
         if "u" in flags:
@@ -909,6 +909,90 @@ def run_ncu_points(args):
                 e1.record()
                 torch.cuda.synchronize()
             print(f"{name} M={M} {label}: {e0.elapsed_time(e1) * 1e3:.1f} us (eager, second of 2 calls)", flush=True)
+
+
+def run_sustained(args):
+    """`--sustained name:M[,name:M...]`: throughput under SUSTAINED load (each candidate runs back
+    to back for ~1.5 s, so the 1 kW power cap, not the burst clock, sets the SM clock; then the
+    next ~40 ms are timed), candidates interleaved over three rounds:
+      * swiglu_mlp (fused), swiglu_mlp_unfused,
+      * CONTEXT ONLY: the vendor GEMM (torch.matmul -> cuBLAS) on the same A and the
+        concatenated [K, 2N] weights -- the same 4MNK FLOP, WITHOUT the activation, writing
+        twice the output.  It is what MEASURED_PEAKS.json's bf16 figures are made of, measured
+        here on the same box, shape, data and protocol.  Not part of the product path.
+    Also repeated with all-zero operands (same kernels, minimal switching power): when the two
+    agree there, what separates them on random data is energy per FLOP, not schedule.
+    Writes gpurun_out/sustained.md."""
+    import torch
+    from paper_2607_02521_b200 import binding as B, inputs
+    import pynvml
+    pynvml.nvmlInit()
+    h = pynvml.nvmlDeviceGetHandleByIndex(0)
+    lib = B.load()
+    probe = clock_probe()
+    st = torch.cuda.current_stream().cuda_stream
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    lines = ["| workload | M | operands | candidate | us (3 rounds) | TFLOP/s (median) | SM MHz in kernel | power W |",
+             "|" + "---|" * 8]
+    for spec in args.sustained.split(","):
+        name, M = spec.split(":")[0], int(spec.split(":")[1])
+        table = dict(inputs.SHAPES)
+        table.update(inputs.PAPER_SHAPES)
+        K, N, seed, _ = table[name]
+        fl = flops(M, N, K)
+        for data in ("N(0,1) x N(0,0.02)", "zeros"):
+            g = torch.Generator(device="cuda").manual_seed(seed)
+            if data == "zeros":
+                A = torch.zeros((M, K), device="cuda", dtype=torch.bfloat16)
+                Wcat = torch.zeros((K, 2 * N), device="cuda", dtype=torch.bfloat16)
+            else:
+                A = torch.randn((M, K), device="cuda", generator=g).bfloat16()
+                Wcat = (torch.randn((K, 2 * N), device="cuda", generator=g) * 0.02).bfloat16()
+            W1, W2 = Wcat[:, :N].contiguous(), Wcat[:, N:].contiguous()
+            Y = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
+            GU = torch.empty((M, 2 * N), dtype=torch.bfloat16, device="cuda")
+            ptr = (A.data_ptr(), W1.data_ptr(), W2.data_ptr(), Y.data_ptr(), M, N, K, st)
+            v4 = [v for v in range(B.swiglu_num_variants()) if "x2_512" in B.swiglu_variant_name(v)]
+            cands = {"swiglu_mlp (fused)": lambda: lib.swiglu_mlp(*ptr),
+                     "swiglu_mlp_unfused": lambda: lib.swiglu_mlp_unfused(*ptr),
+                     "context: cuBLAS GEMM A.[W1|W2] (no activation)": lambda: torch.matmul(A, Wcat, out=GU)}
+            if v4 and M > 256:
+                cands["fused, two-pair cluster with W multicast (forced variant)"] = \
+                    lambda: lib.swiglu_mlp_ex(*ptr[:7], None, 0, v4[0], st)
+            res = {k: [] for k in cands}
+            for fn in cands.values():
+                for _ in range(3):
+                    fn()
+            torch.cuda.synchronize()
+            reps = max(4, int(40e-3 / (fl / 1.3e15)))
+            for rnd in range(3):
+                for nm, fn in cands.items():
+                    t_end = time.time() + 1.5
+                    pw = []
+                    while time.time() < t_end:
+                        for _ in range(4):
+                            fn()
+                        torch.cuda.synchronize()
+                        pw.append(pynvml.nvmlDeviceGetPowerUsage(h) / 1e3)
+                    probe.zero_()
+                    e0.record()
+                    for _ in range(reps):
+                        fn()
+                    e1.record()
+                    torch.cuda.synchronize()
+                    res[nm].append((e0.elapsed_time(e1) * 1e3 / reps, read_probe_mhz(), statistics.median(pw)))
+            for nm, v in res.items():
+                us = [x[0] for x in v]
+                mhz = [x[1] for x in v if x[1]]
+                lines.append(f"| {name} | {M} | {data} | {nm} | {', '.join(f'{u:.0f}' for u in us)} | "
+                             f"{fl / statistics.median(us) / 1e6:.0f} | "
+                             f"{statistics.median(mhz):.0f}" + (" |" if mhz else "- |") +
+                             f" {statistics.median(x[2] for x in v):.0f} |")
+                print(lines[-1], flush=True)
+            del A, Wcat, W1, W2, Y, GU
+            torch.cuda.empty_cache()
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    open(os.path.join(ROOT, "gpurun_out", "sustained.md"), "w").write("\n".join(lines) + "\n")
 
 
 def run_sweep(args):
@@ -997,6 +1081,7 @@ def main():
     ap.add_argument("--decode-study", action="store_true")
     ap.add_argument("--fp8", action="store_true")
     ap.add_argument("--ncu-points", default="")
+    ap.add_argument("--sustained", default="")
     args = ap.parse_args()
     from paper_2607_02521_b200.dist import Ranks
     if args.impl == "reference":
@@ -1021,6 +1106,9 @@ def main():
         return
     if args.ncu_points:
         run_ncu_points(args)
+        return
+    if args.sustained:
+        run_sustained(args)
         return
     ranks = Ranks()
     if ranks.world != args.gpus and ranks.rank == 0:

@@ -61,7 +61,7 @@ struct GemmParams {
   float* split_ws;  // [tail tile][CTA of the group][s][256 columns / 4][128 rows] float4 partials
   int* split_ctr;   // [tail tile][CTA of the group] arrival counters, zero between launches
   int early_issue;      // 1: fill the ring before the CTA-wide setup barrier (small grids)
-  int w_evict_first;    // 1: weights are read once (one row of tiles): L2 evict-first loads
+  unsigned long long w_policy, a_policy;  // L2 eviction-priority hints of the weight / A loads
   unsigned long long* clk;  // optional {SM cycles, globaltimer ns} of CTA 0 (swiglu_set_clock_probe)
   float scale_gate, scale_up;  // kOperandsFp8: Gate / Up dequantisation scales (else unused)
 #ifdef SWIGLU_TRACE
@@ -211,7 +211,16 @@ __device__ __forceinline__ float glu_mul(float g, float u) {
 //     scales multiply the fp32 accumulators in the epilogue before the activation.
 enum : int { kWeightsKN = 0, kWeightsNK = 1, kWeightsPacked = 2, kOperandsFp8 = 3 };
 
-template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = kActSilu, int kWMode = kWeightsKN>
+// kPairs = 2 (with kCtaGroup = 2): a cluster of FOUR CTAs = two CTA pairs working on two
+//   vertically adjacent 256-row tiles of the SAME 128 output columns.  Both pairs need the same
+//   W1|W2 tile: each CTA TMA-loads ONE 64-column slab of its matrix and MULTICASTS it to its
+//   counterpart in the other pair, so every weight byte crosses L2 -> SM once per 512 rows
+//   instead of once per 256 (a quarter less L2 -> SM traffic per FLOP, and the two pairs stay
+//   in lock-step, which roughly halves the DRAM re-reads at the 72B shape:
+//   profiles/r02_ncu_summary.md).  Smem-slot reuse is then gated on BOTH pairs' MMAs: the
+//   tcgen05.commit that frees a stage arrives on all four CTAs' empty barriers.
+template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = kActSilu, int kWMode = kWeightsKN,
+          int kPairs = 1>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                    const __grid_constant__ CUtensorMap tmap_b1,
@@ -219,6 +228,9 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                    const __grid_constant__ CUtensorMap tmap_y, const GemmParams p) {
   static_assert(kBN == 128 || (kBN == 64 && kFused && kCtaGroup == 1), "narrow tile: fused 1-CTA");
   static_assert(kWMode != kWeightsPacked || kFused, "packed weights: fused path only");
+  static_assert(kPairs == 1 || (kPairs == 2 && kCtaGroup == 2 && kFused && kBN == 128),
+                "two pairs per cluster: fused 2-CTA 128-column tiles only");
+  constexpr int kClusterCtas = kCtaGroup * kPairs;
   static_assert(kWMode != kOperandsFp8 || kFused, "FP8 operands: fused path only");
   constexpr bool kF8 = (kWMode == kOperandsFp8);
   constexpr bool kWK = (kWMode == kWeightsNK) || kF8;
@@ -245,14 +257,18 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
 
   const uint32_t warp = threadIdx.x >> 5;
   const uint32_t lane = threadIdx.x & 31u;
-  const uint32_t rank = (kCtaGroup == 2) ? cluster_ctarank() : 0u;
-  const int num_groups = gridDim.x / kCtaGroup;  // CTAs (or CTA pairs) sharing the tile list
-  const int group_id = blockIdx.x / kCtaGroup;
+  const uint32_t crank = (kCtaGroup == 2) ? cluster_ctarank() : 0u;  // rank in the cluster
+  const uint32_t rank = crank & 1u;                // rank in the CTA pair (0 = leader)
+  const uint32_t pair = (kPairs == 2) ? crank >> 1 : 0u;
+  const uint16_t pair_mask = (uint16_t)(0x3u << (2u * pair));        // this pair's two CTAs
+  const uint16_t all_mask = (uint16_t)((1u << kClusterCtas) - 1u);   // every CTA of the cluster
+  const int num_groups = gridDim.x / kClusterCtas;  // clusters (or lone CTAs) sharing the tile list
+  const int group_id = blockIdx.x / kClusterCtas;
   const int total_tiles = p.total_tiles;
   const int k_blocks = (p.K + kBKe - 1) / kBKe;
 
-  // A single row of tiles reads every weight byte exactly once: stream it past L2 (evict-first).
-  const uint64_t w_policy = p.w_evict_first ? kEvictFirst : kEvictNormal;
+  // (host: a single row of tiles reads every weight byte exactly once -> evict-first)
+  const uint64_t w_policy = p.w_policy, a_policy = p.a_policy;
   // One k-block of A and B into ring slot s (no waiting here: the caller owns the ring state).
   // w = output columns of the tile (kOutCols, or 64 for a half tile of the last wave).
   auto issue_loads = [&](int s, int kb, int m_base, int n_base, int w) {
@@ -272,7 +288,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       // slab index of (n_base, Gate): tiles of 128 columns hold 4 slabs g0 u0 g1 u1
       const int slab = (n_base >> 7) * 4 + ((n_base >> 6) & 1) * 2;
       if constexpr (kCtaGroup == 1) {
-        tma_load_2d(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
+        tma_load_2d(sa, &tmap_a, fb, k0, m_base, a_policy);
         if (half) {  // g_h | u_h as two single-slab boxes
           tma_load_3d(sb, &tmap_b2, fb, 0, k0, slab, w_policy);
           tma_load_3d(sb + 8192, &tmap_b2, fb, 0, k0, slab + 1, w_policy);
@@ -280,12 +296,20 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           tma_load_3d(sb, &tmap_b1, fb, 0, k0, slab, w_policy);
         }
       } else {
-        tma_load_2d_pair(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
-        if (half) tma_load_3d_pair(sb, &tmap_b2, fb, 0, k0, slab + (int)rank, w_policy);
-        else tma_load_3d_pair(sb, &tmap_b1, fb, 0, k0, slab + 2 * (int)rank, w_policy);
+        tma_load_2d_pair(sa, &tmap_a, fb, k0, m_base, a_policy);
+        if constexpr (kPairs == 2) {
+          // this CTA needs slabs {2 rank, 2 rank + 1}; it fetches slab 2 rank + pair for itself
+          // and its counterpart in the other pair
+          tma_load_3d_pair_mc(sb + 8192u * pair, &tmap_b2, fb, 0, k0, slab + 2 * (int)rank + (int)pair,
+                              (uint16_t)(0x5u << rank), w_policy);
+        } else if (half) {
+          tma_load_3d_pair(sb, &tmap_b2, fb, 0, k0, slab + (int)rank, w_policy);
+        } else {
+          tma_load_3d_pair(sb, &tmap_b1, fb, 0, k0, slab + 2 * (int)rank, w_policy);
+        }
       }
     } else if constexpr (kCtaGroup == 1) {
-      tma_load_2d(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
+      tma_load_2d(sa, &tmap_a, fb, k0, m_base, a_policy);
       if constexpr (kFused) {
         if (kBN == 64 || half) {  // W1 slab | W2 slab
           load_w(sb, &tmap_b1, n_base);
@@ -301,11 +325,18 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
         for (int j = 0; j < 4; ++j) load_w(sb + j * 8192, &tmap_b1, n_base + j * 64);
       }
     } else {
-      tma_load_2d_pair(sa, &tmap_a, fb, k0, m_base, kEvictNormal);
+      tma_load_2d_pair(sa, &tmap_a, fb, k0, m_base, a_policy);
       if constexpr (kFused) {
         const CUtensorMap* tb = (rank == 0) ? &tmap_b1 : &tmap_b2;
-        load_w(sb, tb, n_base);
-        if (!half) load_w(sb + 8192, tb, n_base + 64);
+        if constexpr (kPairs == 2) {
+          // one 64-column slab of this CTA's matrix, for itself and its counterpart
+          const int n = n_base + 64 * (int)pair;
+          tma_load_2d_pair_mc(sb + 8192u * pair, tb, fb, kWK ? k0 : n, kWK ? n : k0,
+                              (uint16_t)(0x5u << rank), w_policy);
+        } else {
+          load_w(sb, tb, n_base);
+          if (!half) load_w(sb + 8192, tb, n_base + 64);
+        }
       } else {
         const int nb = n_base + (int)rank * 128;
         load_w(sb, &tmap_b1, nb);
@@ -329,7 +360,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       prefetch_tensormap(&tmap_y);
       for (int s = 0; s < kStages; ++s) {
         mbar_init(full_bar(s), 1);
-        mbar_init(empty_bar(s), 1);
+        mbar_init(empty_bar(s), kPairs);  // one commit per pair that reads (or fills) the slot
       }
       for (int a = 0; a < 2; ++a) {
         mbar_init(acc_full_bar(a), 1);
@@ -371,7 +402,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     uint32_t ph = (pre == kStages) ? 1u : 0u;
     for (int t = group_id; t < total_tiles; t += num_groups) {
       const TileUnit u = decode_unit<kOutCols>(p, t, k_blocks);
-      const int m_base = (u.tm * kCtaGroup + (int)rank) * BM;
+      const int m_base = ((u.tm * kPairs + (int)pair) * kCtaGroup + (int)rank) * BM;
       for (int kb = (t == group_id) ? u.kb0 + pre : u.kb0; kb < u.kb1; ++kb) {
         mbar_wait(empty_bar(s), ph ^ 1u);
         issue_loads(s, kb, m_base, u.n_base, u.w);
@@ -414,10 +445,10 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           if constexpr (kF8) umma_f8<kCtaGroup>(d_tmem, adesc, bdesc, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
           else umma_bf16<kCtaGroup>(d_tmem, adesc, bdesc, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
         }
-        umma_commit<kCtaGroup>(empty_bar(s));  // smem stage free once these MMAs retire
+        umma_commit<kCtaGroup>(empty_bar(s), all_mask);  // smem stage free once these MMAs retire
         if (++s == kStages) { s = 0; ph ^= 1u; }
       }
-      umma_commit<kCtaGroup>(acc_full_bar(as));  // accumulator complete -> epilogue
+      umma_commit<kCtaGroup>(acc_full_bar(as), pair_mask);  // accumulator complete -> epilogue
       SWIGLU_GEMM_TRACE(8 + it * 8 + 2);
     }
   } else if (warp >= 2) {
@@ -425,14 +456,15 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     const uint32_t q = warp & 3u;  // TMEM lane quarter this warp may read
     const uint32_t row = q * 32u + lane;
     const bool issuer = (threadIdx.x == 64);
-    const uint32_t leader_acc_empty0 = (kCtaGroup == 2) ? mapa_shared(acc_empty_bar(0), 0) : 0u;
+    const uint32_t leader_acc_empty0 =
+        (kCtaGroup == 2) ? mapa_shared(acc_empty_bar(0), crank & ~1u) : 0u;  // the pair leader's
     int it = 0;
     uint32_t chunk_ctr = 0;
     const uint32_t ticket_slot = tmem_slot + 4u;
     for (int t = group_id; t < total_tiles; t += num_groups, ++it) {
       const TileUnit tu = decode_unit<kOutCols>(p, t, k_blocks);
       const int n_base = tu.n_base, w = tu.w;
-      const int m_base = (tu.tm * kCtaGroup + (int)rank) * BM;
+      const int m_base = ((tu.tm * kPairs + (int)pair) * kCtaGroup + (int)rank) * BM;
       const int chunks = kFused ? w / 64 : kChunks;  // 64-column chunks in this tile
       const int as = it & 1;
       const uint32_t aph = (it >> 1) & 1u;

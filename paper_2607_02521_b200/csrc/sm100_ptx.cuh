@@ -135,6 +135,33 @@ __device__ __forceinline__ void tma_load_2d_pair(uint32_t smem_dst, const void* 
       "l"(reinterpret_cast<uint64_t>(tmap)), "r"(leader_bar), "r"(c0), "r"(c1), "l"(policy)
       : "memory");
 }
+// Pair (cta_group::2) load MULTICAST to the CTAs of `cta_mask` (bit i = cluster rank i): the box
+// lands at the same shared-memory offset in each of them and its bytes are credited to the
+// mbarrier at that offset in each destination's pair leader.
+__device__ __forceinline__ void tma_load_2d_pair_mc(uint32_t smem_dst, const void* tmap,
+                                                    uint32_t bar, int32_t c0, int32_t c1,
+                                                    uint16_t cta_mask, uint64_t policy) {
+  const uint32_t leader_bar = bar & 0xFEFFFFFFu;
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes"
+      ".multicast::cluster.L2::cache_hint [%0], [%1, {%4, %5}], [%2], %3, %6;" ::"r"(smem_dst),
+      "l"(reinterpret_cast<uint64_t>(tmap)), "r"(leader_bar), "h"(cta_mask), "r"(c0), "r"(c1),
+      "l"(policy)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_3d_pair_mc(uint32_t smem_dst, const void* tmap,
+                                                    uint32_t bar, int32_t c0, int32_t c1,
+                                                    int32_t c2, uint16_t cta_mask,
+                                                    uint64_t policy) {
+  const uint32_t leader_bar = bar & 0xFEFFFFFFu;
+  asm volatile(
+      "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes"
+      ".multicast::cluster.L2::cache_hint [%0], [%1, {%4, %5, %6}], [%2], %3, %7;" ::"r"(
+          smem_dst),
+      "l"(reinterpret_cast<uint64_t>(tmap)), "r"(leader_bar), "h"(cta_mask), "r"(c0), "r"(c1),
+      "r"(c2), "l"(policy)
+      : "memory");
+}
 // 3-D tile loads (prepacked weights: {64 columns, k, slab}); same completion rules as the 2-D forms.
 __device__ __forceinline__ void tma_load_3d(uint32_t smem_dst, const void* tmap, uint32_t bar,
                                             int32_t c0, int32_t c1, int32_t c2, uint64_t policy) {
@@ -306,14 +333,14 @@ __device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint6
 }
 // Arrive on `bar` when all previously issued tcgen05.mma of this thread have completed.
 // kCtaGroup == 2: arrives on the barrier at that offset in both CTAs of the pair.
+// `mask`: the cluster ranks whose barrier (same offset) is arrived on; default = ranks 0, 1.
 template <int kCtaGroup>
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
+__device__ __forceinline__ void umma_commit(uint32_t bar, uint16_t mask = 0x3) {
   if constexpr (kCtaGroup == 1) {
     asm volatile(
         "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar)
         : "memory");
   } else {
-    const uint16_t mask = 0x3;
     asm volatile(
         "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster"
         ".b64 [%0], %1;" ::"r"(bar),

@@ -56,7 +56,8 @@ enum FusedVariant {
   kFused2Cta = 1,     // 256x128 tile per CTA pair, cta_group::2
   kFusedSmallM = 2,   // swap-AB, split-K over a cluster, for M <= 128
   kFused1CtaN64 = 3,  // 128x64 (Gate|Up) tile per CTA: twice the tiles when N/128 < #SMs
-  kNumFused = 4
+  kFused2Cta4 = 4,    // cluster of 4 = two CTA pairs on a 512x128 super-tile, W tile multicast
+  kNumFused = 5
 };
 enum UnfusedVariant {
   kUnfused1Cta = 0,    // GEMM 128x256 tiles x2 + elementwise
@@ -65,7 +66,8 @@ enum UnfusedVariant {
   kNumUnfused = 3
 };
 const char* const kFusedNames[kNumFused] = {"fused_1cta_128x128", "fused_2cta_256x128",
-                                            "fused_smallm_swapab_splitk", "fused_1cta_128x64"};
+                                            "fused_smallm_swapab_splitk", "fused_1cta_128x64",
+                                            "fused_2cta_x2_512x128_wmcast"};
 const char* const kUnfusedNames[kNumUnfused] = {"unfused_1cta_gemm128x256+silu_mul",
                                                 "unfused_2cta_gemm256x256+silu_mul",
                                                 "unfused_smallm_gateup_gemm+silu_mul"};
@@ -83,6 +85,7 @@ struct Env {
   bool no_pdl = false, no_prefetch = false, no_early = false, no_tail_split = false,
        no_tail_ksplit = false, no_w_evict_first = false, no_tmap_cache = false;
   int smallm_deep = -1;  // -1 automatic, 0 never, 1 whenever it fits
+  int w_policy = -1, a_policy = -1;  // large-M kernel L2 hints: -1 automatic, 0 normal, 1 first, 2 last
 };
 Env g_env;
 std::once_flag g_env_once;
@@ -104,6 +107,8 @@ void load_env() {
   e.no_w_evict_first = env_int("SWIGLU_NO_W_EVICT_FIRST", 0) != 0;
   e.no_tmap_cache = env_int("SWIGLU_NO_TMAP_CACHE", 0) != 0;
   e.smallm_deep = env_int("SWIGLU_SMALLM_DEEP", -1);
+  e.w_policy = env_int("SWIGLU_W_POLICY", -1);
+  e.a_policy = env_int("SWIGLU_A_POLICY", -1);
   g_env = e;
 }
 const Env& env() {
@@ -210,6 +215,7 @@ int set_smem_attrs() {
   CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true, 128, kAct, kWK>, attr, GemmCfg<1>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true, 64, kAct, kWK>, attr, GemmCfg<1, 128>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, true, 128, kAct, kWK>, attr, GemmCfg<2>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, true, 128, kAct, kWK, 2>, attr, GemmCfg<2>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kAct, kWK>, attr, SmallCfg<16>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kAct, kWK>, attr, SmallCfg<32>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kAct, kWK>, attr, SmallCfg<64>::kSmemBytes));
@@ -379,7 +385,8 @@ TailPlan plan_tail(int64_t tiles, int G, int64_t k_blocks, bool fused128, bool h
 }
 
 // ------------------------------------------------------------------ launches
-template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = swiglu::kActSilu, int kWMode = 0>
+template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = swiglu::kActSilu, int kWMode = 0,
+          int kPairs = 1>
 int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void* B2, void* Yout,
                 int64_t M, int64_t N, int64_t K, cudaStream_t stream, void* split_ws = nullptr,
                 float scale_gate = 1.0f, float scale_up = 1.0f) {
@@ -398,7 +405,8 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   if constexpr (kWMode == kOperandsFp8) {
   } else if constexpr (kWMode == kWeightsPacked) {
     // B1 = Wp: one box per stage -- 4 slabs (1-CTA, 128 columns) or 2 (64-column tile; each
-    // CTA of a pair); single-slab boxes for the half tiles of the last wave
+    // CTA of a pair); single-slab boxes for the half tiles of the last wave and for the
+    // multicast loads of the two-pair cluster
     const uint32_t box = (kCtaGroup == 1 && kBN == 128) ? 4 : 2;
     if ((rc = make_tmap_packed(&tb1, B1, K, packed_slabs(N), box))) return rc;
     if ((rc = make_tmap_packed(&tb2, B1, K, packed_slabs(N), 1))) return rc;
@@ -411,7 +419,7 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   using Cfg = GemmCfg<kCtaGroup, kFused ? 2 * kBN : 256>;
   GemmParams p;
   p.M = (int)M; p.N = (int)N; p.K = (int)K;
-  const int rows_per_tile = BM * kCtaGroup;
+  const int rows_per_tile = BM * kCtaGroup * kPairs;
   const int out_cols = kFused ? kBN : 256;
   p.m_tiles = (int)((M + rows_per_tile - 1) / rows_per_tile);
   p.n_tiles = (int)((N + out_cols - 1) / out_cols);
@@ -423,8 +431,34 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   if (gm > p.m_tiles) gm = p.m_tiles;
   p.group_m = (int)gm;
   const int64_t tiles = (int64_t)p.m_tiles * p.n_tiles;
-  const int G = d.sm_count / kCtaGroup;
-  const TailPlan tail = plan_tail(tiles, G, (K + kBKe - 1) / kBKe, kFused && kBN == 128,
+  int G = d.sm_count / (kCtaGroup * kPairs);
+  if constexpr (kPairs == 2) {
+    // clusters of four do not tile every GPC: ask how many can be resident at once
+    static int max_clusters = -1;  // per (instantiation, process); devices of one process are alike
+    if (max_clusters < 0) {
+      cudaLaunchConfig_t q;
+      memset(&q, 0, sizeof q);
+      q.gridDim = dim3((unsigned)d.sm_count / 4 * 4);
+      q.blockDim = dim3(kGemmThreads);
+      q.dynamicSmemBytes = Cfg::kSmemBytes;
+      cudaLaunchAttribute qa[1];
+      qa[0].id = cudaLaunchAttributeClusterDimension;
+      qa[0].val.clusterDim.x = 4;
+      qa[0].val.clusterDim.y = 1;
+      qa[0].val.clusterDim.z = 1;
+      q.attrs = qa;
+      q.numAttrs = 1;
+      int n = 0;
+      if (cudaOccupancyMaxActiveClusters(&n, gemm_swiglu_kernel<kCtaGroup, kFused, kBN, kAct, kWMode, kPairs>, &q) !=
+              cudaSuccess || n < 1) {
+        cudaGetLastError();
+        n = d.sm_count / 4;
+      }
+      max_clusters = n;
+    }
+    if (G > max_clusters) G = max_clusters;
+  }
+  const TailPlan tail = plan_tail(tiles, G, (K + kBKe - 1) / kBKe, kFused && kBN == 128 && kPairs == 1,
                                   split_ws != nullptr && d.sm_count <= 160);
   p.wide_tiles = (int)tail.wide;
   p.total_tiles = (int)tail.total;
@@ -434,7 +468,13 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   const int groups = (int)(tail.total < G ? tail.total : G);
   // one tile per CTA (a short, HBM-bound call): fill the TMA ring before the setup barrier
   p.early_issue = (kCtaGroup == 1 && kFused && tiles <= groups && tail.ksplit == 0 && !env().no_early);
-  p.w_evict_first = (p.m_tiles == 1 && !env().no_w_evict_first);
+  {
+    const uint64_t pol[3] = {sm100::kEvictNormal, sm100::kEvictFirst, sm100::kEvictLast};
+    p.w_policy = (p.m_tiles == 1 && !env().no_w_evict_first) ? sm100::kEvictFirst : sm100::kEvictNormal;
+    p.a_policy = sm100::kEvictNormal;
+    if (env().w_policy >= 0 && env().w_policy < 3) p.w_policy = pol[env().w_policy];
+    if (env().a_policy >= 0 && env().a_policy < 3) p.a_policy = pol[env().a_policy];
+  }
   p.clk = g_clk.load(std::memory_order_relaxed);
   p.scale_gate = scale_gate;
   p.scale_up = scale_up;
@@ -444,7 +484,7 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
 
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof cfg);
-  cfg.gridDim = dim3((unsigned)(groups * kCtaGroup));
+  cfg.gridDim = dim3((unsigned)(groups * kCtaGroup * kPairs));
   cfg.blockDim = dim3(kGemmThreads);
   cfg.dynamicSmemBytes = Cfg::kSmemBytes;
   cfg.stream = stream;
@@ -452,7 +492,7 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   int na = 0;
   if (kCtaGroup == 2) {
     attrs[na].id = cudaLaunchAttributeClusterDimension;
-    attrs[na].val.clusterDim.x = 2;
+    attrs[na].val.clusterDim.x = 2 * kPairs;
     attrs[na].val.clusterDim.y = 1;
     attrs[na].val.clusterDim.z = 1;
     ++na;
@@ -464,8 +504,8 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   }
   cfg.attrs = attrs;
   cfg.numAttrs = na;
-  CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_swiglu_kernel<kCtaGroup, kFused, kBN, kAct, kWMode>, ta,
-                              tb1, tb2, ty, p));
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_swiglu_kernel<kCtaGroup, kFused, kBN, kAct, kWMode, kPairs>,
+                              ta, tb1, tb2, ty, p));
   return SWIGLU_OK;
 }
 
@@ -697,6 +737,7 @@ int launch_fused_l(const DeviceState& d, int variant, const void* A, const void*
     case kFused2Cta: return launch_gemm<2, true, 128, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream, split_ws);
     case kFusedSmallM: return launch_smallm<kAct, kWK>(d, A, W1, W2, Y, nullptr, M, N, K, stream);
     case kFused1CtaN64: return launch_gemm<1, true, 64, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
+    case kFused2Cta4: return launch_gemm<2, true, 128, kAct, kWK, 2>(d, A, W1, W2, Y, M, N, K, stream);
   }
   return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
 }
@@ -972,6 +1013,8 @@ static int run_fp8(const void* A8, const void* W1, const void* W2, void* Y, int6
       return launch_smallm<kActSilu, kOperandsFp8>(*d, A8, W1, W2, Y, nullptr, M, N, K, stream, 0, sg, su);
     case kFused1CtaN64:
       return launch_gemm<1, true, 64, kActSilu, kOperandsFp8>(*d, A8, W1, W2, Y, M, N, K, stream, nullptr, sg, su);
+    case kFused2Cta4:
+      return launch_gemm<2, true, 128, kActSilu, kOperandsFp8, 2>(*d, A8, W1, W2, Y, M, N, K, stream, nullptr, sg, su);
   }
   return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
 }

@@ -42,7 +42,7 @@ SHAPES = [(1, 128, 128), (7, 136, 80), (16, 4864, 896), (33, 264, 208), (100, 11
           (128, 4864, 896), (129, 264, 208), (300, 1160, 336), (513, 392, 1104), (2560, 1032, 144)]
 
 
-@pytest.mark.parametrize("variant", [-1, 0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [-1, 0, 1, 2, 3, 4])
 @pytest.mark.parametrize("M,N,K", SHAPES)
 def test_fp8_every_variant_on_odd_shapes(variant, M, N, K):
     if variant == 2 and M > 128:

@@ -60,7 +60,7 @@ SHAPES = [(1, 128, 64), (7, 136, 72), (16, 4864, 896), (33, 264, 200), (100, 116
           (128, 4864, 896), (129, 264, 200), (300, 1160, 328), (513, 392, 1096), (2560, 1032, 72)]
 
 
-@pytest.mark.parametrize("variant", [-1, 0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [-1, 0, 1, 2, 3, 4])
 @pytest.mark.parametrize("M,N,K", SHAPES)
 def test_packed_fused_every_variant(variant, M, N, K):
     if variant == 2 and M > 128:

@@ -84,7 +84,8 @@ ODD_SHAPES = [
     (1, 128, 64), (7, 136, 72), (16, 384, 896), (127, 128, 64), (128, 4864, 896),
     (129, 264, 200), (300, 1160, 328), (513, 392, 1096),
 ]
-VARIANTS = [("fused", 0), ("fused", 1), ("fused", 3), ("unfused", 0), ("unfused", 1), ("unfused", 2)]
+VARIANTS = [("fused", 0), ("fused", 1), ("fused", 3), ("fused", 4), ("unfused", 0), ("unfused", 1),
+            ("unfused", 2)]
 
 
 @pytest.mark.parametrize("kind,variant", VARIANTS)
@@ -192,6 +193,21 @@ def test_k_split_is_planned_only_where_it_pays():
     assert ws(16, 4864, 896, -1) == 0        # decode kernel reduces on chip
 
 
+@pytest.mark.parametrize("M,N,K", [(512, 128, 64), (1024, 1160, 328), (769, 392, 1096), (2560, 1032, 200),
+                                   (4096, 4864, 896), (300, 136, 72)])
+def test_two_pair_cluster_multicast_variant(M, N, K):
+    """a3': the cluster of four (two CTA pairs on a 512 x 128 super-tile, each weight slab
+    TMA-multicast to both pairs): even and odd counts of 256-row tiles (the second pair of the
+    last super-tile then works entirely out of range), ragged N and K, many tiles per cluster.
+    Bit-identical to the plain 2-CTA kernel: same tiles, same k order, same epilogue."""
+    A, W1, W2 = inputs.make_case(M, N, K, seed=470 + M + N + K, std=0.05)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+    y4 = run("fused", 4, A, W1, W2)
+    assert_parity(y4, y_ref, ("2x2cta", M, N, K))
+    assert np.array_equal(y4, run("fused", 1, A, W1, W2))
+    assert np.array_equal(y4, run("fused", 4, A, W1, W2))
+
+
 def test_small_m_variant_rejects_large_m():
     A, W1, W2 = inputs.make_case(129, 128, 64, seed=1)
     with pytest.raises(B.SwigluError) as e:
@@ -285,7 +301,7 @@ ACTS = ["gelu", "gelu_tanh", "relu"]
 
 
 @pytest.mark.parametrize("act", ACTS)
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("M,N,K", [(16, 392, 328), (100, 1160, 200), (128, 4864, 896)])
 def test_other_gated_activations_every_fused_variant(act, variant, M, N, K):
     """GeGLU (erf and tanh forms) and ReGLU through every fused kernel, std chosen so Gate
@@ -346,7 +362,7 @@ def test_elementwise_stage_other_activations(act):
     assert_parity(host(dY), y_ref, ("act_mul", act))
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("M,N,K", [(1, 128, 64), (16, 392, 328), (100, 1160, 200), (128, 4864, 896),
                                    (7, 136, 72)])
 def test_nk_weight_layout_every_fused_variant(variant, M, N, K):
