@@ -871,7 +871,8 @@ def run_ncu_points(args):
     """`--ncu-points name:M[:u][,name:M...]`: the kernels behind the per-point claims, launched
     eagerly so that `ncu -k regex:... --set full` can capture them one by one: per point one
     warm-up call and one more of swiglu_mlp (":u" adds swiglu_mlp_unfused, ":p" the prepacked
-    form, ":8" the FP8 form).  Weight copies rotate as in the timed runs (cold L2).  Prints one
+    form, ":8" the FP8 form, ":v" -- as labelled CONTEXT only -- the vendor GEMM torch.matmul(A,
+    [W1|W2]) on the same operands).  Weight copies rotate as in the timed runs (cold L2).  Prints one
     line per point with the CUDA-event time of the last call -- NOT a bench value when run
     under a profiler."""
     import torch
@@ -901,6 +902,14 @@ def run_ncu_points(args):
             A8, W18, W28 = (torch.from_numpy(x).cuda() for x in (A8h, W1h, W2h))
             fns.append(("fp8", lambda a, w1, w2, y, m, n, k, st, _t=(A8, W18, W28, sg, su): lib.swiglu_mlp_fp8(
                 _t[0].data_ptr(), _t[1].data_ptr(), _t[2].data_ptr(), y, m, n, k, _t[3], _t[4], st)))
+        if "v" in flags:
+            Wcat = torch.cat([wl.W1[0], wl.W2[0]], dim=1).contiguous()
+            GU = torch.empty((M, 2 * wl.N), dtype=torch.bfloat16, device="cuda")
+
+            def vendor(a, w1, w2, y, m, n, k, st, _w=Wcat, _o=GU, _a=wl.A[0]):
+                torch.matmul(_a[:m], _w, out=_o)
+                return 0
+            fns.append(("context: vendor GEMM", vendor))
         for label, fn in fns:
             for i in range(2):
                 torch.cuda.synchronize()
@@ -980,14 +989,16 @@ def run_sustained(args):
                         fn()
                     e1.record()
                     torch.cuda.synchronize()
-                    res[nm].append((e0.elapsed_time(e1) * 1e3 / reps, read_probe_mhz(), statistics.median(pw)))
+                    res[nm].append((e0.elapsed_time(e1) * 1e3 / reps,
+                                    None if nm.startswith("context") else read_probe_mhz(),
+                                    statistics.median(pw)))
             for nm, v in res.items():
                 us = [x[0] for x in v]
                 mhz = [x[1] for x in v if x[1]]
                 lines.append(f"| {name} | {M} | {data} | {nm} | {', '.join(f'{u:.0f}' for u in us)} | "
                              f"{fl / statistics.median(us) / 1e6:.0f} | "
-                             f"{statistics.median(mhz):.0f}" + (" |" if mhz else "- |") +
-                             f" {statistics.median(x[2] for x in v):.0f} |")
+                             f"{(f'{statistics.median(mhz):.0f}' if mhz else '-')} | "
+                             f"{statistics.median([x[2] for x in v]):.0f} |")
                 print(lines[-1], flush=True)
             del A, Wcat, W1, W2, Y, GU
             torch.cuda.empty_cache()
