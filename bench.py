@@ -496,12 +496,17 @@ def run_reference(args, ranks):
     ms = 1e3 * sum(times) / len(times)
     value = fl / (ms * 1e-3) / 1e12
     sample = f"{rows} rows x all N columns of {name} per step (fp64 CPU oracle)"
+    from paper_2607_02521_b200 import inputs
+    table = dict(inputs.SHAPES)
+    table.update(inputs.PAPER_SHAPES)
+    K, N, _, Ms = table[name]
+    workload = f"{name}: K={K}, N={N}, one swiglu_mlp call per M in {sorted(Ms, reverse=True)}"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": round(value, 6), "unit": UNIT,
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": round(ms, 3), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": name, "sample": sample},
+        "config": {"workload": workload, "sample": sample},
         "cpu_baseline": {"value": round(value, 6), "unit": UNIT, "cores": used,
                          "kind": "oracle", "sample": sample},
         "e2e": {"value": round(value, 6), "unit": UNIT, "h2d_bytes_per_step": 0,

@@ -61,23 +61,3 @@ class Ranks:
         if self.dist is not None:
             self.dist.destroy_process_group()
             self.dist = None
-
-
-def rank_seed_offset(rank: int) -> int:
-    """Each rank draws its OWN batch of rows (weights are replicated): rows of rank r are the
-    slice [r*M, (r+1)*M) of the shape's activation stream, so N ranks process N*M distinct
-    rows of the same workload."""
-    return int(rank)
-
-
-def shard_rows(total_rows: int, world: int, rank: int):
-    """Contiguous, balanced row ranges for splitting ONE global batch across ranks (the
-    strong-scaling form; rows are independent, Eq. 1-3 act row-wise)."""
-    base, extra = divmod(int(total_rows), int(world))
-    lo = rank * base + min(rank, extra)
-    return lo, lo + base + (1 if rank < extra else 0)
-
-
-def whole_job_throughput(units_per_rank: float, world: int, slowest_seconds: float) -> float:
-    """value = units all ranks processed / max-over-ranks time."""
-    return units_per_rank * world / slowest_seconds
