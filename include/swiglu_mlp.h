@@ -141,12 +141,15 @@ int swiglu_glu_mlp_layout(const void* A, const void* W1, const void* W2, void* Y
  * single columns for its Epilogue Visitor Tree; the unit that matters on sm_100a is the
  * 64-column slab (one 128-byte swizzled TMA box row = one UMMA operand atom), so W_fused is
  *
- *     Wp[t][s][k][c]   t < ceil(N/128) column tiles, s in {g0, u0, g1, u1}, k < K, c < 64
- *                    = W1[k][128 t + 64 (s>>1) + c]  for s even (Gate slabs)
- *                    = W2[k][128 t + 64 (s>>1) + c]  for s odd  (Up slabs)
- *                    = 0 for columns >= N                         (bf16, dense, slab-major)
+ *     Wp[t][s][k][c]   t < ceil(N/128) column tiles, s in {g0, u0, g1, u1}, k < Kp, c < 64
+ *                    = W1[k][128 t + 64 (s>>1) + c]  for s even (Gate slabs), k < K
+ *                    = W2[k][128 t + 64 (s>>1) + c]  for s odd  (Up slabs), k < K
+ *                    = 0 for columns >= N and for the padding rows K <= k < Kp   (bf16, slab-major)
  *
- * i.e. swiglu_packed_weight_bytes(N, K) = 2 * K * pad128(N) * 2 bytes.  One 3-D TMA box then
+ * Kp = K + 8 if K/8 is even, else K + 16: the padding makes the slab pitch Kp * 128 B an odd
+ * number of KiB, which spreads the slabs over the memory channels (with K = 5120 the unpadded
+ * 640 KiB pitch cost 10 % at decode sizes).  swiglu_packed_weight_bytes(N, K) =
+ * 4 * ceil(N/128) * Kp * 128 bytes.  One 3-D TMA box then
  * brings a whole Gate|Up stage (instead of four boxes from two tensors), every 8 KB slab block is
  * contiguous in HBM, and the accumulator columns come out as g0 u0 g1 u1.
  *

@@ -13,6 +13,7 @@ from .oracle import (  # noqa: F401
     build,
     e4m3_to_f64,
     max_threads,
+    pack_rows,
     pack_weights,
     silu,
     swiglu_oracle,

@@ -59,6 +59,7 @@ def _load():
         lib.swiglu_oracle_fp8_rows.argtypes = [p, p, p, p, p, i64, i64, i64, i64, ctypes.c_double,
                                                ctypes.c_double, ctypes.c_int]
         lib.swiglu_oracle_fp8_rows.restype = ctypes.c_int
+        lib.swiglu_oracle_pack_rows.argtypes, lib.swiglu_oracle_pack_rows.restype = [i64], i64
         lib.swiglu_oracle_pack.argtypes = [p, p, p, i64, i64]
         lib.swiglu_oracle_pack.restype = ctypes.c_int
         lib.swiglu_oracle_max_threads.argtypes = []
@@ -142,14 +143,20 @@ def swiglu_oracle_rows(A_bits, W1_bits, W2_bits, rows, nthreads: int = 0, act=0)
     return Y, int(used)
 
 
+def pack_rows(K: int) -> int:
+    """Rows per slab of the W_fused buffer (K plus its padding rows)."""
+    return int(_load().swiglu_oracle_pack_rows(int(K)))
+
+
 def pack_weights(W1_bits, W2_bits):
     """The one-time W_fused interleave (swiglu_oracle.c
-    swiglu_oracle_pack): uint16 [ceil(N/128), 4, K, 64] from W1, W2 [K, N] bit patterns."""
+    swiglu_oracle_pack): uint16 [ceil(N/128), 4, Kp, 64] from W1, W2 [K, N] bit patterns, Kp = K
+    plus 8 or 16 zero padding rows per slab (pack_rows)."""
     W1_bits = np.ascontiguousarray(W1_bits)
     K, N = W1_bits.shape
     W1 = _bits(W1_bits, (K, N), "W1")
     W2 = _bits(W2_bits, (K, N), "W2")
-    Wp = np.empty(((N + 127) // 128, 4, K, 64), dtype=np.uint16)
+    Wp = np.empty(((N + 127) // 128, 4, pack_rows(K), 64), dtype=np.uint16)
     if _load().swiglu_oracle_pack(_ptr(W1), _ptr(W2), _ptr(Wp), N, K) != 0:
         raise RuntimeError("swiglu_oracle_pack rejected its arguments")
     return Wp

@@ -262,26 +262,33 @@ int swiglu_oracle_fp8_rows(const uint8_t* A, const uint8_t* W1, const uint8_t* W
  * tile.  The paper does not print the layout; the reading taken (R18) interleaves
  * 64-column slabs inside 128-column tiles:
  *
- *     Wp[t][s][k][c],  t < ceil(N/128), s in {0,1,2,3} = {gate 0, up 0, gate 1, up 1}, c < 64
- *       = W1[k][128 t + 64 (s/2) + c]   if s is even
- *       = W2[k][128 t + 64 (s/2) + c]   if s is odd
- *       = 0                             where that column is >= N
+ *     Wp[t][s][k][c],  t < ceil(N/128), s in {0,1,2,3} = {gate 0, up 0, gate 1, up 1},
+ *                      k < Kp, c < 64
+ *       = W1[k][128 t + 64 (s/2) + c]   if s is even and k < K
+ *       = W2[k][128 t + 64 (s/2) + c]   if s is odd and k < K
+ *       = 0                             where that column is >= N, or k >= K (padding rows)
+ *
+ * Kp = K + 8 if ceil(K/8) is even, else K + 16: every slab carries 8 or 16 rows of zero padding
+ * so that the distance between slabs, Kp x 128 bytes, is an odd number of KiB (address spread
+ * over the memory channels; not part of the method, only of the buffer's geometry).
  *
  * Pure index work on 16-bit patterns, written as the definition: one loop per index.
  * Pins (tests/test_oracle_pack_pins.py): every (k, n) of W1 and of W2 appears exactly once, at
  * the stated position (checked by an independent inverse walk), padding is zero, a tiny case
  * written out by hand in tests/golden/.
  */
+int64_t swiglu_oracle_pack_rows(int64_t K) { return K + ((((K + 7) / 8) % 2 == 0) ? 8 : 16); }
+
 int swiglu_oracle_pack(const uint16_t* W1, const uint16_t* W2, uint16_t* Wp, int64_t N, int64_t K) {
   if (!W1 || !W2 || !Wp || N <= 0 || K <= 0) return -1;
-  const int64_t tiles = (N + 127) / 128;
+  const int64_t tiles = (N + 127) / 128, Kp = swiglu_oracle_pack_rows(K);
   for (int64_t t = 0; t < tiles; ++t)
     for (int64_t s = 0; s < 4; ++s)
-      for (int64_t k = 0; k < K; ++k)
+      for (int64_t k = 0; k < Kp; ++k)
         for (int64_t c = 0; c < 64; ++c) {
           const int64_t n = 128 * t + 64 * (s / 2) + c;
           const uint16_t* W = (s % 2 == 0) ? W1 : W2;
-          Wp[((t * 4 + s) * K + k) * 64 + c] = (n < N) ? W[k * N + n] : (uint16_t)0;
+          Wp[((t * 4 + s) * Kp + k) * 64 + c] = (n < N && k < K) ? W[k * N + n] : (uint16_t)0;
         }
   return 0;
 }

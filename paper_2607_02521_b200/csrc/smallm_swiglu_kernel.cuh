@@ -395,26 +395,27 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
 // One-time weight prepack (Kernel-2's "one-time preprocessing
 // step" that interleaves W1 and W2; here at 64-column slab granularity, the unit a 128-byte
 // swizzled TMA box and a UMMA operand atom share).
-//   Wp[t][s][k][c], t = n-tile of 128 columns, s in {g0,u0,g1,u1}, k < K, c < 64:
-//     = W{1 if s even else 2}[k][128 t + 64 (s >> 1) + c]      (0 beyond column N)
+//   Wp[t][s][k][c], t = n-tile of 128 columns, s in {g0,u0,g1,u1}, k < Kp, c < 64:
+//     = W{1 if s even else 2}[k][128 t + 64 (s >> 1) + c]      (0 beyond column N or row K)
+//   Kp = K + 8 or 16 padding rows per slab (an odd number of KiB between slabs: address spread).
 // Index work only: each output element is a copy of one input element.
 // ---------------------------------------------------------------------------------------
 template <bool kWK>
 __global__ void __launch_bounds__(256)
 pack_weights_kernel(const uint16_t* __restrict__ W1, const uint16_t* __restrict__ W2,
-                    uint16_t* __restrict__ Wp, int N, int K, long long total_vec) {
+                    uint16_t* __restrict__ Wp, int N, int K, int Kp, long long total_vec) {
   const long long stride = (long long)gridDim.x * blockDim.x;
   for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < total_vec; v += stride) {
     // v indexes 8-element (16-byte) groups of Wp: [slab][k][c8], c8 < 8
     const int c8 = (int)(v & 7);
     const long long row = v >> 3;
-    const int k = (int)(row % K);
-    const long long slab = row / K;
+    const int k = (int)(row % Kp);
+    const long long slab = row / Kp;
     const int s = (int)(slab & 3);
     const int n = (int)(slab >> 2) * 128 + (s >> 1) * 64 + c8 * 8;
     const uint16_t* W = (s & 1) ? W2 : W1;
     uint4 out = make_uint4(0u, 0u, 0u, 0u);
-    if (n < N) {  // N % 8 == 0: the 8 columns are in range together
+    if (n < N && k < K) {  // N % 8 == 0: the 8 columns are in range together
       if constexpr (!kWK) {
         out = __ldg(reinterpret_cast<const uint4*>(W + (long long)k * N + n));
       } else {

@@ -279,9 +279,10 @@ int get_device_state(DeviceState** out) {
 // allocation in between.  Thread-local and direct-mapped, so the hot path takes no lock.
 struct TmapKey {
   const void* base; int64_t d0, d1, d2; uint32_t b0, b1, b2; uint32_t esize;  // 2 = bf16, 1 = fp8
+  int64_t pitch1;  // rows between consecutive d2 slices (>= d1; 0 = dense)
   bool operator==(const TmapKey& o) const {
     return base == o.base && d0 == o.d0 && d1 == o.d1 && d2 == o.d2 && b0 == o.b0 && b1 == o.b1 &&
-           b2 == o.b2 && esize == o.esize;
+           b2 == o.b2 && esize == o.esize && pitch1 == o.pitch1;
   }
 };
 struct TmapSlot { bool used = false; TmapKey key; CUtensorMap map; };
@@ -295,7 +296,7 @@ int encode_tmap(CUtensorMap* out, const TmapKey& k) {
   const cuuint32_t rank = k.d2 ? 3 : 2;
   const cuuint64_t dims[3] = {(cuuint64_t)k.d0, (cuuint64_t)k.d1, (cuuint64_t)k.d2};
   const cuuint64_t strides[2] = {(cuuint64_t)k.d0 * k.esize,
-                                 (cuuint64_t)k.d0 * k.esize * (cuuint64_t)k.d1};
+                                 (cuuint64_t)k.d0 * k.esize * (cuuint64_t)(k.pitch1 ? k.pitch1 : k.d1)};
   const cuuint32_t box[3] = {k.b0, k.b1, k.b2};
   const cuuint32_t elem[3] = {1, 1, 1};
   const CUresult r =
@@ -314,7 +315,7 @@ int cached_tmap(CUtensorMap* out, const TmapKey& key) {
   uint64_t h = (uint64_t)(uintptr_t)key.base * 0x9E3779B97F4A7C15ull;
   h ^= ((uint64_t)key.d0 * 0xC2B2AE3D27D4EB4Full) ^ ((uint64_t)key.d1 * 0x165667B19E3779F9ull) ^
        ((uint64_t)key.d2 * 0x27D4EB2F165667C5ull) ^ ((uint64_t)key.b1 << 7) ^ ((uint64_t)key.b2 << 17) ^
-       ((uint64_t)key.esize << 27);
+       ((uint64_t)key.esize << 27) ^ ((uint64_t)key.pitch1 << 31);
   TmapSlot& slot = t_tmaps[(h >> 40) & (kTmapSlots - 1)];
   if (slot.used && slot.key == key) {
     ++t_tmap_hits;
@@ -333,17 +334,22 @@ int cached_tmap(CUtensorMap* out, const TmapKey& key) {
 // 2-D tensor [outer, inner] (inner contiguous), box = box_outer x box_inner.
 int make_tmap(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
               uint32_t box_inner, uint32_t box_outer) {
-  return cached_tmap(out, TmapKey{base, inner, outer, 0, box_inner, box_outer, 0, 2});
+  return cached_tmap(out, TmapKey{base, inner, outer, 0, box_inner, box_outer, 0, 2, 0});
 }
 // FP8 (1-byte) 2-D tensor [outer, inner]: a box row is 128 elements = 128 bytes.
 int make_tmap_u8(CUtensorMap* out, const void* base, int64_t inner, int64_t outer,
                  uint32_t box_outer) {
-  return cached_tmap(out, TmapKey{base, inner, outer, 0, 128, box_outer, 0, 1});
+  return cached_tmap(out, TmapKey{base, inner, outer, 0, 128, box_outer, 0, 1, 0});
 }
-// Prepacked weights Wp[slab][k][64]: {64, K, slabs}, box = 64 x 64 x box_slabs.
+// Rows per slab of the prepacked buffer: K plus 8 or 16 padding rows, chosen so that the slab
+// pitch (rows x 128 B) is an ODD number of KiB.  With a power-of-two-ish pitch (K = 5120: 640 KiB)
+// the CTAs of a decode call -- all at the same k, one slab pitch apart -- walk addresses that
+// collide in the L2 / HBM channel hash (32B decode: 94 us packed vs 84 us plain before the pad).
+inline int64_t packed_rows(int64_t K) { return K + ((((K + 7) / 8) % 2 == 0) ? 8 : 16); }
+// Prepacked weights Wp[slab][packed_rows(K)][64]: {64, K, slabs}, box = 64 x 64 x box_slabs.
 int make_tmap_packed(CUtensorMap* out, const void* base, int64_t K, int64_t slabs,
                      uint32_t box_slabs) {
-  return cached_tmap(out, TmapKey{base, 64, K, slabs, 64, 64, box_slabs, 2});
+  return cached_tmap(out, TmapKey{base, 64, K, slabs, 64, 64, box_slabs, 2, packed_rows(K)});
 }
 inline int64_t packed_slabs(int64_t N) { return 4 * ((N + 127) / 128); }
 
@@ -786,7 +792,7 @@ int run_fused(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
   if (rc) return rc;
   if (layout == kWeightsPacked && M > 0) {
     // the packed buffer is 2 * K * pad128(N) elements: re-check aliasing against its real size
-    const int64_t pb = 2 * K * ((N + 127) / 128 * 128) * 2;
+    const int64_t pb = packed_slabs(N) * packed_rows(K) * 128;
     if (overlaps(Y, M * N * 2, W1, pb)) return fail(SWIGLU_ERR_ALIASING, "Y overlaps Wp");
   }
   if (act < 0 || act >= swiglu::kNumActs)
@@ -928,7 +934,7 @@ int swiglu_glu_mlp_ex(const void* A, const void* W1, const void* W2, void* Y, in
 
 size_t swiglu_packed_weight_bytes(int64_t N, int64_t K) {
   if (N <= 0 || K <= 0 || (N % 8) || (K % 8)) return 0;
-  return (size_t)2 * (size_t)K * (size_t)((N + 127) / 128 * 128) * 2;
+  return (size_t)packed_slabs(N) * (size_t)packed_rows(K) * 128;
 }
 
 int swiglu_pack_weights(const void* W1, const void* W2, void* Wp, int64_t N, int64_t K,
@@ -950,10 +956,10 @@ int swiglu_pack_weights(const void* W1, const void* W2, void* Wp, int64_t N, int
   if (blocks > cap) blocks = cap;
   if (weight_layout == SWIGLU_WEIGHTS_NK)
     swiglu::pack_weights_kernel<true><<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(
-        (const uint16_t*)W1, (const uint16_t*)W2, (uint16_t*)Wp, (int)N, (int)K, total_vec);
+        (const uint16_t*)W1, (const uint16_t*)W2, (uint16_t*)Wp, (int)N, (int)K, (int)packed_rows(K), total_vec);
   else
     swiglu::pack_weights_kernel<false><<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(
-        (const uint16_t*)W1, (const uint16_t*)W2, (uint16_t*)Wp, (int)N, (int)K, total_vec);
+        (const uint16_t*)W1, (const uint16_t*)W2, (uint16_t*)Wp, (int)N, (int)K, (int)packed_rows(K), total_vec);
   CUDA_TRY(cudaGetLastError());
   return SWIGLU_OK;
 }

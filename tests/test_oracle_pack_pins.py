@@ -22,7 +22,9 @@ def test_every_weight_appears_exactly_once_at_the_stated_place(K, N):
     W1, W2 = tagged(K, N, 0), tagged(K, N, 1)
     Wp = oracle.pack_weights(W1, W2)
     T = (N + 127) // 128
-    assert Wp.shape == (T, 4, K, 64)
+    Kp = oracle.pack_rows(K)
+    assert Wp.shape == (T, 4, Kp, 64)
+    assert Kp - K in (8, 16) and (Kp * 128 // 1024) % 2 == 1 if K % 8 == 0 else Kp > K
     # inverse walk, written from the other side: for each (matrix, k, n) say where it must be
     seen = np.zeros(Wp.shape, dtype=bool)
     for which, W in ((0, W1), (1, W2)):
@@ -35,7 +37,7 @@ def test_every_weight_appears_exactly_once_at_the_stated_place(K, N):
                 assert not seen[t, s, k, c]
                 seen[t, s, k, c] = True
     assert seen.sum() == 2 * K * N
-    assert np.all(Wp[~seen] == 0)                     # padding columns (n >= N) are zero
+    assert np.all(Wp[~seen] == 0)                     # padding columns (n >= N) and rows (k >= K)
 
 
 def test_gate_and_up_columns_of_one_output_share_a_tile():
@@ -47,8 +49,16 @@ def test_gate_and_up_columns_of_one_output_share_a_tile():
     for n in range(N):
         t, r = divmod(n, 128)
         half, c = divmod(r, 64)
-        assert np.array_equal(Wp[t, 2 * half, :, c], W1[:, n])
-        assert np.array_equal(Wp[t, 2 * half + 1, :, c], W2[:, n])
+        assert np.array_equal(Wp[t, 2 * half, :K, c], W1[:, n])
+        assert np.array_equal(Wp[t, 2 * half + 1, :K, c], W2[:, n])
+
+
+@pytest.mark.parametrize("K,Kp", [(8, 24), (16, 24), (896, 904), (1536, 1544), (3584, 3592), (5120, 5128),
+                                  (8192, 8200), (72, 88)])
+def test_slab_pitch_is_an_odd_number_of_kib(K, Kp):
+    """Hand-computed: K/8 even -> +8 rows, K/8 odd -> +16, so Kp * 128 B is an odd multiple of 1 KiB."""
+    assert oracle.pack_rows(K) == Kp
+    assert (Kp * 128) % 1024 == 0 and ((Kp * 128) // 1024) % 2 == 1
 
 
 def test_hand_written_example():

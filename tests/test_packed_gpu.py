@@ -26,7 +26,7 @@ def host(t):
 def pack(W1, W2, layout=B.WEIGHTS_KN):
     K, N = W1.shape
     nbytes = B.swiglu_packed_weight_bytes(N, K)
-    assert nbytes == 2 * K * ((N + 127) // 128 * 128) * 2
+    assert nbytes == 4 * ((N + 127) // 128) * oracle.pack_rows(K) * 64 * 2
     buf = torch.full((nbytes // 2 + 64,), -21846, dtype=torch.int16, device="cuda")  # + guard
     Wp = buf[:nbytes // 2]
     if layout == B.WEIGHTS_KN:

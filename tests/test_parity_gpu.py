@@ -181,6 +181,38 @@ def test_last_wave_k_split(variant, M, N, K, force_s, swiglu_env):
     assert_parity(call(), y_ref, ("no split", variant, M, N, K))
 
 
+def test_last_wave_k_split_with_other_operand_modes(swiglu_env):
+    """The K split of the last wave runs in every operand mode of the large-M kernels: [N,K]
+    weights, prepacked weights (accumulator columns g0 u0 g1 u1) and FP8 operands (k-blocks of
+    128 elements)."""
+    swiglu_env("SWIGLU_TAIL_KSPLIT", 3)
+    M, N, K = 2560, 1032, 1024
+    A, W1, W2 = inputs.make_case(M, N, K, seed=480, std=0.05)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+    dA = dev(A)
+    for variant in (0, 1):
+        assert B.swiglu_workspace_bytes(M, N, K, unfused=False, variant=variant) > 0
+        dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+        B.swiglu_glu_mlp_layout(dA, dev(np.ascontiguousarray(W1.T)), dev(np.ascontiguousarray(W2.T)), dY,
+                                "silu", B.WEIGHTS_NK, variant=variant)
+        torch.cuda.synchronize()
+        assert_parity(host(dY), y_ref, ("k-split nk", variant))
+        Wp = torch.empty(B.swiglu_packed_weight_bytes(N, K) // 2, dtype=torch.int16, device="cuda")
+        B.swiglu_pack_weights(dev(W1), dev(W2), Wp, N, K)
+        dY.fill_(float("nan"))
+        B.swiglu_glu_mlp_packed(dA, Wp, dY, "silu", variant)
+        torch.cuda.synchronize()
+        assert_parity(host(dY), y_ref, ("k-split packed", variant))
+    A8, W18, W28, sg, su = inputs.make_fp8_case(M, N, 2048, seed=481, std=0.05)
+    y8, _ = oracle.swiglu_oracle_fp8(A8, W18, W28, sg, su)
+    for variant in (0, 1):
+        dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+        B.swiglu_mlp_fp8(torch.from_numpy(A8).cuda(), torch.from_numpy(W18).cuda(),
+                         torch.from_numpy(W28).cuda(), dY, sg, su, variant)
+        torch.cuda.synchronize()
+        assert_parity(host(dY), y8, ("k-split fp8", variant))
+
+
 def test_k_split_is_planned_only_where_it_pays():
     """Host-side plan: a sparse last wave of a big-K shape gets a workspace (= a
     K split); full waves, dense tails and short K do not."""
