@@ -28,8 +28,13 @@ using namespace sm100;
 constexpr int BM = 128;      // rows of A / Y per CTA
 constexpr int BK = 64;       // k per pipeline stage: 64 bf16 = one 128-byte swizzle row
 constexpr int UMMA_K = 16;   // k per tcgen05.mma (kind::f16)
-constexpr int kEpiWarps = 4;
-constexpr int kGemmThreads = 64 + 32 * kEpiWarps;  // warp 0 TMA, warp 1 MMA, warps 2-5 epilogue
+// Eight epilogue warps: two per TMEM lane quarter (a warp may only read lanes 32*(warp%4)..+31).
+// Of every 64-column output chunk, warps 2-5 take columns [0,32) and warps 6-9 columns [32,64):
+// two warps per SM sub-partition hide each other's TMEM-load / MUFU latencies, which halves the
+// drain time of a tile (3.6 -> 1.8 us per 128x128 tile) wherever it is exposed: one tile per CTA
+// near the ridge, the last tile of every call, FP8 at small K.
+constexpr int kEpiWarps = 8;
+constexpr int kGemmThreads = 64 + 32 * kEpiWarps;  // warp 0 TMA, warp 1 MMA, warps 2-9 epilogue
 constexpr int kOutBufBytes = BM * 64 * 2;          // one 64-column bf16 output chunk (16 KB)
 
 // kUmmaN = accumulator columns per tile: 256 (fused: Gate 128 | Up 128; unfused: 256 plain
@@ -455,6 +460,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     // ================================================================ epilogue
     const uint32_t q = warp & 3u;  // TMEM lane quarter this warp may read
     const uint32_t row = q * 32u + lane;
+    const uint32_t eg = (warp - 2u) >> 2;  // 0: columns [0,32) of each 64-column chunk, 1: [32,64)
     const bool issuer = (threadIdx.x == 64);
     const uint32_t leader_acc_empty0 =
         (kCtaGroup == 2) ? mapa_shared(acc_empty_bar(0), crank & ~1u) : 0u;  // the pair leader's
@@ -483,7 +489,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           const size_t slot = (size_t)tu.tail * kCtaGroup + rank;
           float4* part = reinterpret_cast<float4*>(p.split_ws) + (slot * S + tu.krank) * (size_t)(64 * BM);
 #pragma unroll 1
-          for (int cc = 0; cc < UMMA_N / 32; ++cc) {
+          for (int cc = (int)eg; cc < UMMA_N / 32; cc += 2) {
             uint32_t v[32];
             tmem_ld_32x32b_x32(tacc + cc * 32, v);
             tmem_ld_wait();
@@ -520,8 +526,8 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
         // the TMA store that last read this buffer (2 chunks ago) must have finished reading
         if (issuer) tma_store_wait_read<1>();
         named_bar_sync(1, kEpiWarps * 32);
-#pragma unroll
-        for (int c = 0; c < 2; ++c) {
+        {
+          const int c = (int)eg;  // this warp's half of the chunk
           uint32_t packed[16];
           if constexpr (kFused) {
             uint32_t g[32], u[32];
@@ -573,7 +579,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
             for (int j = 0; j < 16; ++j)
               packed[j] = pack_bf16x2_rn(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
           }
-          if (h == chunks - 1 && c == 1 && split_src == nullptr) {
+          if (h == chunks - 1 && split_src == nullptr) {
             // last TMEM read of this tile is done: hand the accumulator stage back to the MMA
             tcgen05_fence_before();
             __syncwarp();
