@@ -966,13 +966,14 @@ def run_sustained(args):
             Y = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
             GU = torch.empty((M, 2 * N), dtype=torch.bfloat16, device="cuda")
             ptr = (A.data_ptr(), W1.data_ptr(), W2.data_ptr(), Y.data_ptr(), M, N, K, st)
-            v4 = [v for v in range(B.swiglu_num_variants()) if "x2_512" in B.swiglu_variant_name(v)]
             cands = {"swiglu_mlp (fused)": lambda: lib.swiglu_mlp(*ptr),
                      "swiglu_mlp_unfused": lambda: lib.swiglu_mlp_unfused(*ptr),
                      "context: cuBLAS GEMM A.[W1|W2] (no activation)": lambda: torch.matmul(A, Wcat, out=GU)}
-            if v4 and M > 256:
-                cands["fused, two-pair cluster with W multicast (forced variant)"] = \
-                    lambda: lib.swiglu_mlp_ex(*ptr[:7], None, 0, v4[0], st)
+            auto = B.swiglu_selected_variant(M, N, K)
+            for v in range(B.swiglu_num_variants()):   # the other large-M kernels, forced
+                vn = B.swiglu_variant_name(v)
+                if M > 256 and v != auto and vn.startswith("fused_2cta"):
+                    cands[f"forced variant {vn}"] = (lambda _v=v: lib.swiglu_mlp_ex(*ptr[:7], None, 0, _v, st))
             res = {k: [] for k in cands}
             for fn in cands.values():
                 for _ in range(3):

@@ -40,14 +40,14 @@ constexpr int kOutBufBytes = BM * 64 * 2;          // one 64-column bf16 output 
 // kUmmaN = accumulator columns per tile: 256 (fused: Gate 128 | Up 128; unfused: 256 plain
 // columns) or, for the narrow fused tile used when N/128 tiles cannot fill the GPU,
 // 128 (Gate 64 | Up 64).
-template <int kCtaGroup, int kUmmaN = 256>
+template <int kCtaGroup, int kUmmaN = 256, int kMB = 1>
 struct GemmCfg {
   static constexpr int kBColsPerCta = kUmmaN / kCtaGroup;
-  static constexpr int kABytes = BM * BK * 2;            // 16 KB
+  static constexpr int kABytes = kMB * BM * BK * 2;      // 16 KB per 128-row block of A
   static constexpr int kBBytes = kBColsPerCta * BK * 2;  // 32 KB (1-CTA) / 16 KB (2-CTA, narrow)
   static constexpr int kStageBytes = kABytes + kBBytes;
   static constexpr int kStages = (kStageBytes >= 48 * 1024) ? 4 : 6;
-  static constexpr int kTmemCols = 2 * kUmmaN;           // 2 accumulator stages
+  static constexpr int kTmemCols = 2 * kUmmaN;           // 2 accumulator stages (kMB = 2: 2 row blocks)
   static constexpr int kBarBytes = 1024;
   // +1024: slack to align the dynamic smem base to 1024 B (128-byte swizzle atoms)
   static constexpr int kSmemBytes = kStages * kStageBytes + 2 * kOutBufBytes + kBarBytes + 1024;
@@ -63,6 +63,7 @@ struct GemmParams {
                     // >= 2), or two 64-column half tiles (tail_ksplit == 0)
   int total_tiles;  // schedule slots: wide_tiles + units of the cut tiles
   int tail_ksplit;  // s: K-ranges per tile of the last wave (0 = no K split)
+  int skew;         // kMB = 2: k-blocks row block 0 runs ahead of block 1 at tile boundaries
   float* split_ws;  // [tail tile][CTA of the group][s][256 columns / 4][128 rows] float4 partials
   int* split_ctr;   // [tail tile][CTA of the group] arrival counters, zero between launches
   int early_issue;      // 1: fill the ring before the CTA-wide setup barrier (small grids)
@@ -224,8 +225,21 @@ enum : int { kWeightsKN = 0, kWeightsNK = 1, kWeightsPacked = 2, kOperandsFp8 = 
 //   in lock-step, which roughly halves the DRAM re-reads at the 72B shape:
 //   profiles/r02_ncu_summary.md).  Smem-slot reuse is then gated on BOTH pairs' MMAs: the
 //   tcgen05.commit that frees a stage arrives on all four CTAs' empty barriers.
+//
+// kMB = 2 (with kCtaGroup = 2, one pair per cluster): a 512-row x 128-column SUPER TILE per CTA
+//   pair.  Each CTA stages TWO 128-row blocks of A per k-block (rows +0 and +256 of the tile) next
+//   to its half of the W1|W2 tile, and the leader issues two M = 256 MMAs per k-step that share the
+//   weight operand: accumulator region 0 (TMEM columns [0,256)) = rows [0,256) of the tile, region
+//   1 (columns [256,512)) = rows [256,512).  Per FLOP a quarter less L2 -> SM traffic than the
+//   256-row pair tile (96 KB instead of 128 KB per 512x128x64 block), on every SM and with no
+//   cluster wider than the pair.  All of TMEM then belongs to ONE tile, so the epilogue is hidden
+//   by SKEWING the row blocks at tile boundaries instead of by a second accumulator stage: the
+//   last L k-blocks of a tile run "block 0 first" (region 0 is complete L k-blocks early and
+//   drains under block 1's last MMAs) and the first L k-blocks of the next tile likewise (block
+//   0's MMAs run while region 1 still drains).  L <= ring depth; in between the blocks interleave
+//   so that the ring keeps its full prefetch depth.
 template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = kActSilu, int kWMode = kWeightsKN,
-          int kPairs = 1>
+          int kPairs = 1, int kMB = 1>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                    const __grid_constant__ CUtensorMap tmap_b1,
@@ -235,6 +249,8 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   static_assert(kWMode != kWeightsPacked || kFused, "packed weights: fused path only");
   static_assert(kPairs == 1 || (kPairs == 2 && kCtaGroup == 2 && kFused && kBN == 128),
                 "two pairs per cluster: fused 2-CTA 128-column tiles only");
+  static_assert(kMB == 1 || (kMB == 2 && kCtaGroup == 2 && kFused && kBN == 128 && kPairs == 1),
+                "two row blocks per CTA: fused 2-CTA 128-column tiles, one pair per cluster");
   constexpr int kClusterCtas = kCtaGroup * kPairs;
   static_assert(kWMode != kOperandsFp8 || kFused, "FP8 operands: fused path only");
   constexpr bool kF8 = (kWMode == kOperandsFp8);
@@ -242,7 +258,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   constexpr bool kPacked = (kWMode == kWeightsPacked);
   constexpr int kBKe = kF8 ? 128 : BK;            // elements of k per stage (128-byte rows)
   constexpr int UMMA_N = kFused ? 2 * kBN : 256;  // accumulator columns per tile
-  using Cfg = GemmCfg<kCtaGroup, UMMA_N>;
+  using Cfg = GemmCfg<kCtaGroup, UMMA_N, kMB>;
   constexpr int kStages = Cfg::kStages;
   constexpr int kTmemCols = Cfg::kTmemCols;
   constexpr int kOutCols = kFused ? kBN : 256;  // output columns per tile
@@ -302,6 +318,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
         }
       } else {
         tma_load_2d_pair(sa, &tmap_a, fb, k0, m_base, a_policy);
+        if constexpr (kMB == 2) tma_load_2d_pair(sa + BM * BK * 2, &tmap_a, fb, k0, m_base + 2 * BM, a_policy);
         if constexpr (kPairs == 2) {
           // this CTA needs slabs {2 rank, 2 rank + 1}; it fetches slab 2 rank + pair for itself
           // and its counterpart in the other pair
@@ -331,6 +348,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       }
     } else {
       tma_load_2d_pair(sa, &tmap_a, fb, k0, m_base, a_policy);
+      if constexpr (kMB == 2) tma_load_2d_pair(sa + BM * BK * 2, &tmap_a, fb, k0, m_base + 2 * BM, a_policy);
       if constexpr (kFused) {
         const CUtensorMap* tb = (rank == 0) ? &tmap_b1 : &tmap_b2;
         if constexpr (kPairs == 2) {
@@ -407,7 +425,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     uint32_t ph = (pre == kStages) ? 1u : 0u;
     for (int t = group_id; t < total_tiles; t += num_groups) {
       const TileUnit u = decode_unit<kOutCols>(p, t, k_blocks);
-      const int m_base = ((u.tm * kPairs + (int)pair) * kCtaGroup + (int)rank) * BM;
+      const int m_base = ((u.tm * kPairs * kMB + (int)pair) * kCtaGroup + (int)rank) * BM;
       for (int kb = (t == group_id) ? u.kb0 + pre : u.kb0; kb < u.kb1; ++kb) {
         mbar_wait(empty_bar(s), ph ^ 1u);
         issue_loads(s, kb, m_base, u.n_base, u.w);
@@ -421,6 +439,62 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
             : idesc_bf16_f32(BM * kCtaGroup, UMMA_N, /*a_mn=*/false, /*b_mn=*/!kWK);
     constexpr uint32_t idesc_half = kF8 ? idesc_e4m3_f32(BM * kCtaGroup, 128)
                                         : idesc_bf16_f32(BM * kCtaGroup, 128, false, !kWK);
+    if constexpr (kMB == 2) {
+      // Two row blocks per tile sharing every weight stage; block 0 runs ahead of block 1 by up
+      // to L k-blocks at the head and at the tail of a tile (see the kernel comment).  s0 / s1:
+      // ring slots of the next k-block of block 0 / block 1; a slot is waited for once (block 0
+      // always touches it first) and freed by the commit after block 1's MMAs.
+      int s0 = 0, s1 = 0;
+      uint32_t ph0 = 0;
+      int it = 0;
+      const int L = min(max(p.skew, 1), kStages);
+      for (int t = group_id; t < total_tiles; t += num_groups, ++it) {
+        const uint32_t aph = it & 1u;
+        const TileUnit u = decode_unit<kOutCols>(p, t, k_blocks);
+        const int n = u.kb1 - u.kb0;
+        const int H = min(L, n), T = min(L, n - H);
+        int i0 = 0, i1 = 0;
+        auto mma_block = [&](int b, int s, bool first) {
+          const uint32_t sa = smem_a(s) + b * (BM * BK * 2), sb = smem_b(s);
+          const uint32_t d_tmem = tmem_base + b * UMMA_N;
+#pragma unroll
+          for (int k = 0; k < BK / UMMA_K; ++k) {
+            const uint64_t adesc = smem_desc_sw128(sa + k * (UMMA_K * 2), 16, 1024);
+            const uint64_t bdesc = kWK ? smem_desc_sw128(sb + k * (UMMA_K * 2), 16, 1024)
+                                       : smem_desc_sw128(sb + k * (UMMA_K * 128), 8192, 1024);
+            if constexpr (kF8) umma_f8<kCtaGroup>(d_tmem, adesc, bdesc, idesc_full, (!first || k > 0) ? 1u : 0u);
+            else umma_bf16<kCtaGroup>(d_tmem, adesc, bdesc, idesc_full, (!first || k > 0) ? 1u : 0u);
+          }
+        };
+        auto do0 = [&]() {
+          mbar_wait(full_bar(s0), ph0);
+          tcgen05_fence_after();
+          mma_block(0, s0, i0 == 0);
+          ++i0;
+          if (++s0 == kStages) { s0 = 0; ph0 ^= 1u; }
+        };
+        auto do1 = [&]() {
+          mma_block(1, s1, i1 == 0);
+          umma_commit<kCtaGroup>(empty_bar(s1), all_mask);  // both blocks have read the stage
+          ++i1;
+          if (++s1 == kStages) s1 = 0;
+        };
+        mbar_wait(acc_empty_bar(0), aph ^ 1u);  // region 0 drained
+        tcgen05_fence_after();
+        for (int i = 0; i < H; ++i) do0();
+        if (T == 0) umma_commit<kCtaGroup>(acc_full_bar(0), pair_mask);  // the whole K range fitted the head
+        mbar_wait(acc_empty_bar(1), aph ^ 1u);  // region 1 drained
+        tcgen05_fence_after();
+        for (int i = 0; i < H; ++i) do1();
+        for (int i = n - H - T; i > 0; --i) { do0(); do1(); }
+        if (T > 0) {
+          for (int i = 0; i < T; ++i) do0();
+          umma_commit<kCtaGroup>(acc_full_bar(0), pair_mask);  // region 0 complete: drains under block 1's tail
+          for (int i = 0; i < T; ++i) do1();
+        }
+        umma_commit<kCtaGroup>(acc_full_bar(1), pair_mask);
+      }
+    } else {
     int s = 0;
     uint32_t ph = 0;
     int it = 0;
@@ -456,6 +530,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       umma_commit<kCtaGroup>(acc_full_bar(as), pair_mask);  // accumulator complete -> epilogue
       SWIGLU_GEMM_TRACE(8 + it * 8 + 2);
     }
+    }
   } else if (warp >= 2) {
     // ================================================================ epilogue
     const uint32_t q = warp & 3u;  // TMEM lane quarter this warp may read
@@ -470,10 +545,12 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     for (int t = group_id; t < total_tiles; t += num_groups, ++it) {
       const TileUnit tu = decode_unit<kOutCols>(p, t, k_blocks);
       const int n_base = tu.n_base, w = tu.w;
-      const int m_base = ((tu.tm * kPairs + (int)pair) * kCtaGroup + (int)rank) * BM;
       const int chunks = kFused ? w / 64 : kChunks;  // 64-column chunks in this tile
-      const int as = it & 1;
-      const uint32_t aph = (it >> 1) & 1u;
+#pragma unroll 1
+      for (int mb = 0; mb < kMB; ++mb) {  // accumulator regions of the tile (kMB = 2: two row blocks)
+      const int m_base = ((tu.tm * kPairs * kMB + (int)pair) * kCtaGroup + (int)rank) * BM + mb * (2 * BM);
+      const int as = (kMB == 2) ? mb : (it & 1);
+      const uint32_t aph = (kMB == 2) ? (it & 1u) : ((it >> 1) & 1u);
       mbar_wait(acc_full_bar(as), aph);
       if (issuer) SWIGLU_GEMM_TRACE(8 + it * 8 + 3);
       tcgen05_fence_after();
@@ -602,6 +679,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           tma_store_2d(&tmap_y, obuf, n_base + h * 64, m_base);  // OOB rows/cols are clipped
           tma_store_commit();
         }
+      }
       }
       if (issuer) SWIGLU_GEMM_TRACE(8 + it * 8 + 4);
     }

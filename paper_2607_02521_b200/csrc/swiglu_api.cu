@@ -57,7 +57,8 @@ enum FusedVariant {
   kFusedSmallM = 2,   // swap-AB, split-K over a cluster, for M <= 128
   kFused1CtaN64 = 3,  // 128x64 (Gate|Up) tile per CTA: twice the tiles when N/128 < #SMs
   kFused2Cta4 = 4,    // cluster of 4 = two CTA pairs on a 512x128 super-tile, W tile multicast
-  kNumFused = 5
+  kFused2CtaMB2 = 5,  // 512x128 super-tile per CTA pair: two row blocks share each weight stage
+  kNumFused = 6
 };
 enum UnfusedVariant {
   kUnfused1Cta = 0,    // GEMM 128x256 tiles x2 + elementwise
@@ -67,7 +68,8 @@ enum UnfusedVariant {
 };
 const char* const kFusedNames[kNumFused] = {"fused_1cta_128x128", "fused_2cta_256x128",
                                             "fused_smallm_swapab_splitk", "fused_1cta_128x64",
-                                            "fused_2cta_x2_512x128_wmcast"};
+                                            "fused_2cta_x2_512x128_wmcast",
+                                            "fused_2cta_512x128_2rowblocks"};
 const char* const kUnfusedNames[kNumUnfused] = {"unfused_1cta_gemm128x256+silu_mul",
                                                 "unfused_2cta_gemm256x256+silu_mul",
                                                 "unfused_smallm_gateup_gemm+silu_mul"};
@@ -82,6 +84,7 @@ int env_int(const char* name, int dflt) {
 // getenv.  All default to "off" / "automatic".
 struct Env {
   int variant = -1, unfused_variant = -1, ksplit = 0, group_m = 0, host_chunks = 4, tail_ksplit = 0;
+  int skew = 4;  // super-tile kernel: k-blocks row block 0 leads block 1 at tile boundaries
   bool no_pdl = false, no_prefetch = false, no_early = false, no_tail_split = false,
        no_tail_ksplit = false, no_w_evict_first = false, no_tmap_cache = false;
   int smallm_deep = -1;  // -1 automatic, 0 never, 1 whenever it fits
@@ -107,6 +110,7 @@ void load_env() {
   e.no_w_evict_first = env_int("SWIGLU_NO_W_EVICT_FIRST", 0) != 0;
   e.no_tmap_cache = env_int("SWIGLU_NO_TMAP_CACHE", 0) != 0;
   e.smallm_deep = env_int("SWIGLU_SMALLM_DEEP", -1);
+  e.skew = env_int("SWIGLU_SKEW", 4);
   e.w_policy = env_int("SWIGLU_W_POLICY", -1);
   e.a_policy = env_int("SWIGLU_A_POLICY", -1);
   g_env = e;
@@ -216,6 +220,7 @@ int set_smem_attrs() {
   CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, true, 64, kAct, kWK>, attr, GemmCfg<1, 128>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, true, 128, kAct, kWK>, attr, GemmCfg<2>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, true, 128, kAct, kWK, 2>, attr, GemmCfg<2>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, true, 128, kAct, kWK, 1, 2>, attr, GemmCfg<2, 256, 2>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kAct, kWK>, attr, SmallCfg<16>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kAct, kWK>, attr, SmallCfg<32>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kAct, kWK>, attr, SmallCfg<64>::kSmemBytes));
@@ -392,7 +397,7 @@ TailPlan plan_tail(int64_t tiles, int G, int64_t k_blocks, bool fused128, bool h
 
 // ------------------------------------------------------------------ launches
 template <int kCtaGroup, bool kFused, int kBN = 128, int kAct = swiglu::kActSilu, int kWMode = 0,
-          int kPairs = 1>
+          int kPairs = 1, int kMB = 1>
 int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void* B2, void* Yout,
                 int64_t M, int64_t N, int64_t K, cudaStream_t stream, void* split_ws = nullptr,
                 float scale_gate = 1.0f, float scale_up = 1.0f) {
@@ -422,10 +427,10 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
     if ((rc = make_tmap(&tb2, kFused ? B2 : B1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
   }
   if ((rc = make_tmap(&ty, Yout, N, M, 64, 128))) return rc;
-  using Cfg = GemmCfg<kCtaGroup, kFused ? 2 * kBN : 256>;
+  using Cfg = GemmCfg<kCtaGroup, kFused ? 2 * kBN : 256, kMB>;
   GemmParams p;
   p.M = (int)M; p.N = (int)N; p.K = (int)K;
-  const int rows_per_tile = BM * kCtaGroup * kPairs;
+  const int rows_per_tile = BM * kCtaGroup * kPairs * kMB;
   const int out_cols = kFused ? kBN : 256;
   p.m_tiles = (int)((M + rows_per_tile - 1) / rows_per_tile);
   p.n_tiles = (int)((N + out_cols - 1) / out_cols);
@@ -464,11 +469,12 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
     }
     if (G > max_clusters) G = max_clusters;
   }
-  const TailPlan tail = plan_tail(tiles, G, (K + kBKe - 1) / kBKe, kFused && kBN == 128 && kPairs == 1,
+  const TailPlan tail = plan_tail(tiles, G, (K + kBKe - 1) / kBKe, kFused && kBN == 128 && kPairs == 1 && kMB == 1,
                                   split_ws != nullptr && d.sm_count <= 160);
   p.wide_tiles = (int)tail.wide;
   p.total_tiles = (int)tail.total;
   p.tail_ksplit = tail.ksplit;
+  p.skew = env().skew;
   p.split_ctr = (int*)split_ws;
   p.split_ws = split_ws ? (float*)((char*)split_ws + kSplitCtrBytes) : nullptr;
   const int groups = (int)(tail.total < G ? tail.total : G);
@@ -510,7 +516,7 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   }
   cfg.attrs = attrs;
   cfg.numAttrs = na;
-  CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_swiglu_kernel<kCtaGroup, kFused, kBN, kAct, kWMode, kPairs>,
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_swiglu_kernel<kCtaGroup, kFused, kBN, kAct, kWMode, kPairs, kMB>,
                               ta, tb1, tb2, ty, p));
   return SWIGLU_OK;
 }
@@ -744,6 +750,7 @@ int launch_fused_l(const DeviceState& d, int variant, const void* A, const void*
     case kFusedSmallM: return launch_smallm<kAct, kWK>(d, A, W1, W2, Y, nullptr, M, N, K, stream);
     case kFused1CtaN64: return launch_gemm<1, true, 64, kAct, kWK>(d, A, W1, W2, Y, M, N, K, stream);
     case kFused2Cta4: return launch_gemm<2, true, 128, kAct, kWK, 2>(d, A, W1, W2, Y, M, N, K, stream);
+    case kFused2CtaMB2: return launch_gemm<2, true, 128, kAct, kWK, 1, 2>(d, A, W1, W2, Y, M, N, K, stream);
   }
   return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
 }
@@ -1021,6 +1028,8 @@ static int run_fp8(const void* A8, const void* W1, const void* W2, void* Y, int6
       return launch_gemm<1, true, 64, kActSilu, kOperandsFp8>(*d, A8, W1, W2, Y, M, N, K, stream, nullptr, sg, su);
     case kFused2Cta4:
       return launch_gemm<2, true, 128, kActSilu, kOperandsFp8, 2>(*d, A8, W1, W2, Y, M, N, K, stream, nullptr, sg, su);
+    case kFused2CtaMB2:
+      return launch_gemm<2, true, 128, kActSilu, kOperandsFp8, 1, 2>(*d, A8, W1, W2, Y, M, N, K, stream, nullptr, sg, su);
   }
   return fail(SWIGLU_ERR_UNSUPPORTED, "unknown fused variant %d", variant);
 }
