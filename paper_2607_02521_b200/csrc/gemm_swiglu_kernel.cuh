@@ -64,6 +64,7 @@ struct GemmParams {
   int total_tiles;  // schedule slots: wide_tiles + units of the cut tiles
   int tail_ksplit;  // s: K-ranges per tile of the last wave (0 = no K split)
   int skew;         // kMB = 2: k-blocks row block 0 runs ahead of block 1 at tile boundaries
+  int tail_div;     // kMB = 2: units per super tile of the last partial wave (1, 2 or 4)
   float* split_ws;  // [tail tile][CTA of the group][s][256 columns / 4][128 rows] float4 partials
   int* split_ctr;   // [tail tile][CTA of the group] arrival counters, zero between launches
   int early_issue;      // 1: fill the ring before the CTA-wide setup barrier (small grids)
@@ -139,11 +140,33 @@ __device__ __forceinline__ void decode_tile_w(const GemmParams& p, int t, int& t
 // discuss the wave quantisation this removes).
 struct TileUnit {
   int tm, n_base, w, kb0, kb1, tail, krank;
+  int mb0, nmb;  // kMB = 2: first 256-row block of the super tile this unit covers, and how many
 };
-template <int kOutCols>
+template <int kOutCols, int kMB = 1>
 __device__ __forceinline__ TileUnit decode_unit(const GemmParams& p, int t, int k_blocks) {
   TileUnit u;
-  u.kb0 = 0; u.kb1 = k_blocks; u.tail = -1; u.krank = 0;
+  u.kb0 = 0; u.kb1 = k_blocks; u.tail = -1; u.krank = 0; u.mb0 = 0; u.nmb = 1;
+  if constexpr (kMB == 2) {
+    // Super tiles (two row blocks); the last partial wave is cut into p.tail_div units per
+    // tile: 2 = its two row blocks, 4 = row blocks x 64-column halves, each run by one CTA pair
+    // with a single accumulator region.  A super tile whose second block lies beyond M (ragged
+    // M) is run as one block.
+    int tn;
+    if (t < p.wide_tiles) {
+      decode_tile(p, t, u.tm, tn);
+      u.n_base = tn * kOutCols;
+      u.w = kOutCols;
+      u.nmb = ((u.tm * 4 + 2) * BM < p.M) ? 2 : 1;
+    } else {
+      const int j = t - p.wide_tiles;
+      const int tile = j / p.tail_div, sub = j - tile * p.tail_div;
+      decode_tile(p, p.wide_tiles + tile, u.tm, tn);
+      u.mb0 = sub & 1;
+      u.w = (p.tail_div == 4) ? 64 : kOutCols;
+      u.n_base = tn * kOutCols + ((p.tail_div == 4) ? (sub >> 1) * 64 : 0);
+    }
+    return u;
+  }
   if (t >= p.wide_tiles && p.tail_ksplit >= 2) {
     const int idx = t - p.wide_tiles;
     u.tail = idx / p.tail_ksplit;
@@ -249,8 +272,8 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   static_assert(kWMode != kWeightsPacked || kFused, "packed weights: fused path only");
   static_assert(kPairs == 1 || (kPairs == 2 && kCtaGroup == 2 && kFused && kBN == 128),
                 "two pairs per cluster: fused 2-CTA 128-column tiles only");
-  static_assert(kMB == 1 || (kMB == 2 && kCtaGroup == 2 && kFused && kBN == 128 && kPairs == 1),
-                "two row blocks per CTA: fused 2-CTA 128-column tiles, one pair per cluster");
+  static_assert(kMB == 1 || (kMB == 2 && kCtaGroup == 2 && kBN == 128 && kPairs == 1),
+                "two row blocks per CTA: 2-CTA tiles of 256 accumulator columns, one pair per cluster");
   constexpr int kClusterCtas = kCtaGroup * kPairs;
   static_assert(kWMode != kOperandsFp8 || kFused, "FP8 operands: fused path only");
   constexpr bool kF8 = (kWMode == kOperandsFp8);
@@ -292,11 +315,12 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   const uint64_t w_policy = p.w_policy, a_policy = p.a_policy;
   // One k-block of A and B into ring slot s (no waiting here: the caller owns the ring state).
   // w = output columns of the tile (kOutCols, or 64 for a half tile of the last wave).
-  auto issue_loads = [&](int s, int kb, int m_base, int n_base, int w) {
+  auto issue_loads = [&](int s, int kb, int m_base, int n_base, int w, int nmb = kMB) {
     const bool half = kFused && kBN == 128 && w == 64;
     if (rank == 0) {
       const uint32_t b_bytes = half ? Cfg::kBBytes / 2 : Cfg::kBBytes;
-      mbar_arrive_expect_tx(full_bar(s), (Cfg::kABytes + b_bytes) * kCtaGroup);
+      const uint32_t a_bytes = (kMB == 2 && nmb == 1) ? Cfg::kABytes / 2 : Cfg::kABytes;
+      mbar_arrive_expect_tx(full_bar(s), (a_bytes + b_bytes) * kCtaGroup);
     }
     const int k0 = kb * kBKe;
     const uint32_t sa = smem_a(s), sb = smem_b(s), fb = full_bar(s);
@@ -318,7 +342,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
         }
       } else {
         tma_load_2d_pair(sa, &tmap_a, fb, k0, m_base, a_policy);
-        if constexpr (kMB == 2) tma_load_2d_pair(sa + BM * BK * 2, &tmap_a, fb, k0, m_base + 2 * BM, a_policy);
+        if (kMB == 2 && nmb == 2) tma_load_2d_pair(sa + BM * BK * 2, &tmap_a, fb, k0, m_base + 2 * BM, a_policy);
         if constexpr (kPairs == 2) {
           // this CTA needs slabs {2 rank, 2 rank + 1}; it fetches slab 2 rank + pair for itself
           // and its counterpart in the other pair
@@ -348,7 +372,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       }
     } else {
       tma_load_2d_pair(sa, &tmap_a, fb, k0, m_base, a_policy);
-      if constexpr (kMB == 2) tma_load_2d_pair(sa + BM * BK * 2, &tmap_a, fb, k0, m_base + 2 * BM, a_policy);
+      if (kMB == 2 && nmb == 2) tma_load_2d_pair(sa + BM * BK * 2, &tmap_a, fb, k0, m_base + 2 * BM, a_policy);
       if constexpr (kFused) {
         const CUtensorMap* tb = (rank == 0) ? &tmap_b1 : &tmap_b2;
         if constexpr (kPairs == 2) {
@@ -424,11 +448,11 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     int s = (pre == kStages) ? 0 : pre;
     uint32_t ph = (pre == kStages) ? 1u : 0u;
     for (int t = group_id; t < total_tiles; t += num_groups) {
-      const TileUnit u = decode_unit<kOutCols>(p, t, k_blocks);
-      const int m_base = ((u.tm * kPairs * kMB + (int)pair) * kCtaGroup + (int)rank) * BM;
+      const TileUnit u = decode_unit<kOutCols, kMB>(p, t, k_blocks);
+      const int m_base = ((u.tm * kPairs * kMB + (int)pair + u.mb0) * kCtaGroup + (int)rank) * BM;
       for (int kb = (t == group_id) ? u.kb0 + pre : u.kb0; kb < u.kb1; ++kb) {
         mbar_wait(empty_bar(s), ph ^ 1u);
-        issue_loads(s, kb, m_base, u.n_base, u.w);
+        issue_loads(s, kb, m_base, u.n_base, u.w, u.nmb);
         if (++s == kStages) { s = 0; ph ^= 1u; }
       }
     }
@@ -446,14 +470,12 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       // always touches it first) and freed by the commit after block 1's MMAs.
       int s0 = 0, s1 = 0;
       uint32_t ph0 = 0;
-      int it = 0;
+      uint32_t it0 = 0, it1 = 0;  // uses of accumulator region 0 / 1 so far (barrier phases)
       const int L = min(max(p.skew, 1), kStages);
-      for (int t = group_id; t < total_tiles; t += num_groups, ++it) {
-        const uint32_t aph = it & 1u;
-        const TileUnit u = decode_unit<kOutCols>(p, t, k_blocks);
+      for (int t = group_id; t < total_tiles; t += num_groups) {
+        const TileUnit u = decode_unit<kOutCols, kMB>(p, t, k_blocks);
         const int n = u.kb1 - u.kb0;
-        const int H = min(L, n), T = min(L, n - H);
-        int i0 = 0, i1 = 0;
+        const uint32_t idesc = (u.w == 64) ? idesc_half : idesc_full;
         auto mma_block = [&](int b, int s, bool first) {
           const uint32_t sa = smem_a(s) + b * (BM * BK * 2), sb = smem_b(s);
           const uint32_t d_tmem = tmem_base + b * UMMA_N;
@@ -462,10 +484,30 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
             const uint64_t adesc = smem_desc_sw128(sa + k * (UMMA_K * 2), 16, 1024);
             const uint64_t bdesc = kWK ? smem_desc_sw128(sb + k * (UMMA_K * 2), 16, 1024)
                                        : smem_desc_sw128(sb + k * (UMMA_K * 128), 8192, 1024);
-            if constexpr (kF8) umma_f8<kCtaGroup>(d_tmem, adesc, bdesc, idesc_full, (!first || k > 0) ? 1u : 0u);
-            else umma_bf16<kCtaGroup>(d_tmem, adesc, bdesc, idesc_full, (!first || k > 0) ? 1u : 0u);
+            if constexpr (kF8) umma_f8<kCtaGroup>(d_tmem, adesc, bdesc, idesc, (!first || k > 0) ? 1u : 0u);
+            else umma_bf16<kCtaGroup>(d_tmem, adesc, bdesc, idesc, (!first || k > 0) ? 1u : 0u);
           }
         };
+        if (u.nmb == 1) {
+          // one row block (a unit of the cut last wave, or a ragged last row tile): region 0 only
+          mbar_wait(acc_empty_bar(0), (it0 & 1u) ^ 1u);
+          tcgen05_fence_after();
+          for (int i = 0; i < n; ++i) {
+            mbar_wait(full_bar(s0), ph0);
+            tcgen05_fence_after();
+            mma_block(0, s0, i == 0);
+            umma_commit<kCtaGroup>(empty_bar(s0), all_mask);
+            if (++s0 == kStages) { s0 = 0; ph0 ^= 1u; }
+          }
+          s1 = s0;
+          umma_commit<kCtaGroup>(acc_full_bar(0), pair_mask);
+          ++it0;
+          continue;
+        }
+        const uint32_t aph0 = it0 & 1u, aph1 = it1 & 1u;
+        ++it0; ++it1;
+        const int H = min(L, n), T = min(L, n - H);
+        int i0 = 0, i1 = 0;
         auto do0 = [&]() {
           mbar_wait(full_bar(s0), ph0);
           tcgen05_fence_after();
@@ -479,11 +521,11 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           ++i1;
           if (++s1 == kStages) s1 = 0;
         };
-        mbar_wait(acc_empty_bar(0), aph ^ 1u);  // region 0 drained
+        mbar_wait(acc_empty_bar(0), aph0 ^ 1u);  // region 0 drained
         tcgen05_fence_after();
         for (int i = 0; i < H; ++i) do0();
         if (T == 0) umma_commit<kCtaGroup>(acc_full_bar(0), pair_mask);  // the whole K range fitted the head
-        mbar_wait(acc_empty_bar(1), aph ^ 1u);  // region 1 drained
+        mbar_wait(acc_empty_bar(1), aph1 ^ 1u);  // region 1 drained
         tcgen05_fence_after();
         for (int i = 0; i < H; ++i) do1();
         for (int i = n - H - T; i > 0; --i) { do0(); do1(); }
@@ -540,17 +582,19 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     const uint32_t leader_acc_empty0 =
         (kCtaGroup == 2) ? mapa_shared(acc_empty_bar(0), crank & ~1u) : 0u;  // the pair leader's
     int it = 0;
+    uint32_t reg_phase = 0;  // kMB = 2: bit r = barrier phase of accumulator region r
     uint32_t chunk_ctr = 0;
     const uint32_t ticket_slot = tmem_slot + 4u;
     for (int t = group_id; t < total_tiles; t += num_groups, ++it) {
-      const TileUnit tu = decode_unit<kOutCols>(p, t, k_blocks);
+      const TileUnit tu = decode_unit<kOutCols, kMB>(p, t, k_blocks);
       const int n_base = tu.n_base, w = tu.w;
       const int chunks = kFused ? w / 64 : kChunks;  // 64-column chunks in this tile
 #pragma unroll 1
-      for (int mb = 0; mb < kMB; ++mb) {  // accumulator regions of the tile (kMB = 2: two row blocks)
-      const int m_base = ((tu.tm * kPairs * kMB + (int)pair) * kCtaGroup + (int)rank) * BM + mb * (2 * BM);
+      for (int mb = 0; mb < tu.nmb; ++mb) {  // accumulator regions of the tile (kMB = 2: row blocks)
+      const int m_base = ((tu.tm * kPairs * kMB + (int)pair + tu.mb0 + mb) * kCtaGroup + (int)rank) * BM;
       const int as = (kMB == 2) ? mb : (it & 1);
-      const uint32_t aph = (kMB == 2) ? (it & 1u) : ((it >> 1) & 1u);
+      const uint32_t aph = (kMB == 2) ? ((reg_phase >> mb) & 1u) : ((it >> 1) & 1u);
+      reg_phase ^= 1u << mb;
       mbar_wait(acc_full_bar(as), aph);
       if (issuer) SWIGLU_GEMM_TRACE(8 + it * 8 + 3);
       tcgen05_fence_after();

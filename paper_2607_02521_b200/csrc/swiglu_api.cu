@@ -64,7 +64,8 @@ enum UnfusedVariant {
   kUnfused1Cta = 0,    // GEMM 128x256 tiles x2 + elementwise
   kUnfused2Cta = 1,    // GEMM 256x256 pair tiles x2 + elementwise
   kUnfusedSmallM = 2,  // M <= 128: ONE merged Gate|Up swap-AB split-K GEMM + elementwise
-  kNumUnfused = 3
+  kUnfused2CtaMB2 = 3, // GEMM 512x256 super tiles (two row blocks per CTA) x2 + elementwise
+  kNumUnfused = 4
 };
 const char* const kFusedNames[kNumFused] = {"fused_1cta_128x128", "fused_2cta_256x128",
                                             "fused_smallm_swapab_splitk", "fused_1cta_128x64",
@@ -72,7 +73,8 @@ const char* const kFusedNames[kNumFused] = {"fused_1cta_128x128", "fused_2cta_25
                                             "fused_2cta_512x128_2rowblocks"};
 const char* const kUnfusedNames[kNumUnfused] = {"unfused_1cta_gemm128x256+silu_mul",
                                                 "unfused_2cta_gemm256x256+silu_mul",
-                                                "unfused_smallm_gateup_gemm+silu_mul"};
+                                                "unfused_smallm_gateup_gemm+silu_mul",
+                                                "unfused_2cta_gemm512x256+silu_mul"};
 
 int env_int(const char* name, int dflt) {
   const char* v = getenv(name);
@@ -120,9 +122,35 @@ const Env& env() {
   return g_env;
 }
 
+struct TailPlan { int64_t wide, total; int ksplit; };
+TailPlan plan_tail(int64_t tiles, int G, int64_t k_blocks, bool fused128, bool have_ws);
+int super_tail_div(int64_t tiles, int G, int max_div = 4);
+int64_t super_tail_cost4(int64_t rem, int G, int div);
+
+// Wave efficiency (ideal waves / scheduled waves, in tile times) of the two pair kernels on
+// `pairs` CTA pairs: the 256-row kernel with its last-wave plan, the 512-row super-tile kernel
+// with its cut last wave.
+double wave_eff_pair(int64_t M, int64_t N, int64_t K, int pairs) {
+  const int64_t tiles = ((M + 255) / 256) * ((N + 127) / 128);
+  const TailPlan t = plan_tail(tiles, pairs, (K + 63) / 64, true, true);
+  const int64_t rem = tiles % pairs;
+  double waves = (double)(tiles / pairs);
+  if (rem) waves += t.ksplit >= 2 ? 1.0 / t.ksplit + 0.1 : (t.total > tiles ? 0.5 : 1.0);
+  return (double)tiles / pairs / waves;
+}
+double wave_eff_super(int64_t M, int64_t N, int pairs, int cols = 128) {
+  const int64_t n_tiles = (N + cols - 1) / cols;
+  const int64_t tiles = ((M + 511) / 512) * n_tiles;
+  const int64_t rem = tiles % pairs;
+  double waves = (double)(tiles / pairs);
+  if (rem) waves += super_tail_cost4(rem, pairs, super_tail_div(tiles, pairs, cols == 128 ? 4 : 2)) / 4.0;
+  // a ragged last row tile with one block costs half a tile
+  const double work = (double)((M + 255) / 256) * n_tiles / 2.0;
+  return work / pairs / waves;
+}
+
 // Measured dispatch (table regenerated from bench sweeps).
 int select_fused(int64_t M, int64_t N, int64_t K) {
-  (void)K;
   const int forced = env().variant;
   if (forced >= 0 && forced < kNumFused) {
     if (forced != kFusedSmallM || M <= swiglu::kSmallMMax) return forced;
@@ -139,16 +167,29 @@ int select_fused(int64_t M, int64_t N, int64_t K) {
   if (M <= 32) return kFusedSmallM;
   if (M <= 64) return few_tiles ? kFused1CtaN64 : kFusedSmallM;
   if (M <= 128) return few_tiles ? kFused1CtaN64 : kFused1Cta;
+  // M > 128: a CTA-pair kernel.  The 512-row super tile moves a quarter less data per FLOP and
+  // these calls are power-bound (profiles/r02_variant_sweep_super_tile.md: +1-6 % in short
+  // bursts, +3-5 % under sustained load) -- where each tile's mainloop is long enough to
+  // amortise the skewed tile boundary (K >= 2048: the 1.5B-class shapes are 5 % slower with it)
+  // and the 512-row granularity does not cost more in wave quantisation than it gains.
+  if (M > 512 && K >= 2048 && wave_eff_super(M, N, 74) >= wave_eff_pair(M, N, K, 74) - 0.03)
+    return kFused2CtaMB2;
   return kFused2Cta;
 }
 int select_unfused(int64_t M, int64_t N, int64_t K) {
-  (void)N; (void)K;
   const int forced = env().unfused_variant;
   if (forced >= 0 && forced < kNumUnfused && (forced != kUnfusedSmallM || M <= swiglu::kSmallMMax))
     return forced;
   // Decode sizes: the same swap-AB split-K streaming kernel as the fused path, writing bf16
   // Gate and Up -- so that fused vs unfused compares fusion, not tile shapes.
-  return (M <= 128) ? kUnfusedSmallM : kUnfused2Cta;
+  if (M <= 128) return kUnfusedSmallM;
+  // Large M: the same super-tile rule as the fused path (same mainloop, same power argument).
+  if (M > 512 && K >= 2048) {
+    const int64_t tiles = ((M + 255) / 256) * ((N + 255) / 256), rem = tiles % 74;
+    const double eff_pair = (double)tiles / 74 / (double)(tiles / 74 + (rem ? 1 : 0));
+    if (wave_eff_super(M, N, 74, 256) >= eff_pair - 0.03) return kUnfused2CtaMB2;
+  }
+  return kUnfused2Cta;
 }
 
 // ------------------------------------------------------------------ validation (no CUDA)
@@ -236,6 +277,7 @@ int set_smem_attrs() {
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<128, kActSilu, kWK, true>, attr, SmallCfg<128>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<1, false, 128, kActSilu, kWK>, attr, GemmCfg<1>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, false, 128, kActSilu, kWK>, attr, GemmCfg<2>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(gemm_swiglu_kernel<2, false, 128, kActSilu, kWK, 1, 2>, attr, GemmCfg<2, 256, 2>::kSmemBytes));
   }
   return SWIGLU_OK;
 }
@@ -374,7 +416,19 @@ constexpr int kSplitMinKBlocks = 16;
 constexpr size_t kSplitCtrBytes = 4096;                      // counters: one int per (tile, CTA)
 constexpr size_t kSplitPartialBytes = 256 * 128 * 4;         // one CTA's fp32 accumulators
 constexpr size_t kSplitWsBytes = kSplitCtrBytes + 160 * kSplitPartialBytes;  // up to 160 SMs
-struct TailPlan { int64_t wide, total; int ksplit; };
+// Super-tile kernel: units per tile of the last partial wave (1 = whole tiles, 2 = row blocks,
+// 4 = row blocks x 64-column halves): the coarsest cut that minimises the time of the tail,
+// ceil(rem * div / G) / div tile times.
+int64_t super_tail_cost4(int64_t rem, int G, int div) { return (rem * div + G - 1) / G * (4 / div); }
+int super_tail_div(int64_t tiles, int G, int max_div) {
+  const int64_t rem = tiles % G;
+  if (rem == 0 || env().no_tail_split) return 1;
+  if (env().tail_ksplit == 2 || env().tail_ksplit == max_div) return env().tail_ksplit;  // experiments
+  int best = 1;
+  for (int div = 2; div <= max_div; div *= 2)
+    if (super_tail_cost4(rem, G, div) < super_tail_cost4(rem, G, best)) best = div;
+  return best;
+}
 TailPlan plan_tail(int64_t tiles, int G, int64_t k_blocks, bool fused128, bool have_ws) {
   TailPlan t{tiles, tiles, 0};
   const int64_t rem = tiles % G;
@@ -435,7 +489,9 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   p.m_tiles = (int)((M + rows_per_tile - 1) / rows_per_tile);
   p.n_tiles = (int)((N + out_cols - 1) / out_cols);
   // L2 raster group: keep the slab of A the running CTAs share at <= 32 MiB
-  int64_t gm = (32ll << 20) / ((int64_t)rows_per_tile * K * (kWMode == kOperandsFp8 ? 1 : 2));
+  // (64 MiB for the super-tile kernel: 72B M=8192 sustained, group of 2 / 4 / 8 / 16 super tiles:
+  // 1309 / 1357 / 1367 / 1302 TFLOP/s)
+  int64_t gm = ((kMB == 2 ? 64ll : 32ll) << 20) / ((int64_t)rows_per_tile * K * (kWMode == kOperandsFp8 ? 1 : 2));
   const int forced_gm = env().group_m;
   if (forced_gm > 0) gm = forced_gm;
   if (gm < 1) gm = 1;
@@ -475,9 +531,20 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   p.total_tiles = (int)tail.total;
   p.tail_ksplit = tail.ksplit;
   p.skew = env().skew;
+  p.tail_div = 1;
+  if constexpr (kMB == 2) {
+    // last partial wave of super tiles: cut every tile into its two row blocks, or into row
+    // blocks x 64-column halves, when that many units still fit one wave
+    const int64_t rem = tiles % G;
+    p.tail_div = super_tail_div(tiles, G, kFused ? 4 : 2);  // (a plain GEMM tile has no column halves)
+    if (p.tail_div > 1) {
+      p.wide_tiles = (int)(tiles - rem);
+      p.total_tiles = (int)(tiles - rem + rem * p.tail_div);
+    }
+  }
   p.split_ctr = (int*)split_ws;
   p.split_ws = split_ws ? (float*)((char*)split_ws + kSplitCtrBytes) : nullptr;
-  const int groups = (int)(tail.total < G ? tail.total : G);
+  const int groups = (int)(p.total_tiles < G ? p.total_tiles : G);
   // one tile per CTA (a short, HBM-bound call): fill the TMA ring before the setup barrier
   p.early_issue = (kCtaGroup == 1 && kFused && tiles <= groups && tail.ksplit == 0 && !env().no_early);
   {
@@ -865,6 +932,12 @@ int run_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t 
   } else if (variant == kUnfused1Cta) {
     if ((rc = launch_gemm<1, false, 128, kActSilu, kWeightsNK>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
     if ((rc = launch_gemm<1, false, 128, kActSilu, kWeightsNK>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
+  } else if (variant == kUnfused2CtaMB2 && !layout) {
+    if ((rc = launch_gemm<2, false, 128, kActSilu, kWeightsKN, 1, 2>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
+    if ((rc = launch_gemm<2, false, 128, kActSilu, kWeightsKN, 1, 2>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
+  } else if (variant == kUnfused2CtaMB2) {
+    if ((rc = launch_gemm<2, false, 128, kActSilu, kWeightsNK, 1, 2>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
+    if ((rc = launch_gemm<2, false, 128, kActSilu, kWeightsNK, 1, 2>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
   } else if (!layout) {
     if ((rc = launch_gemm<2, false>(*d, A, W1, W1, G, M, N, K, stream))) return rc;
     if ((rc = launch_gemm<2, false>(*d, A, W2, W2, U, M, N, K, stream))) return rc;
@@ -1014,7 +1087,7 @@ static int run_fp8(const void* A8, const void* W1, const void* W2, void* Y, int6
   DeviceState* d;
   int rc;
   if ((rc = get_device_state(&d))) return rc;
-  if (variant < 0) variant = select_fused(M, N, K);
+  if (variant < 0) variant = select_fused(M, N, K / 2);  // a k-block is 128 one-byte elements
   using namespace swiglu;
   void* split_ws = workspace_for(M, N, K / 2, 0, variant) > 0 ? split_workspace(*d, stream) : nullptr;
   switch (variant) {

@@ -84,8 +84,8 @@ ODD_SHAPES = [
     (1, 128, 64), (7, 136, 72), (16, 384, 896), (127, 128, 64), (128, 4864, 896),
     (129, 264, 200), (300, 1160, 328), (513, 392, 1096),
 ]
-VARIANTS = [("fused", 0), ("fused", 1), ("fused", 3), ("fused", 4), ("unfused", 0), ("unfused", 1),
-            ("unfused", 2)]
+VARIANTS = [("fused", 0), ("fused", 1), ("fused", 3), ("fused", 4), ("fused", 5), ("unfused", 0),
+            ("unfused", 1), ("unfused", 2), ("unfused", 3)]
 
 
 @pytest.mark.parametrize("kind,variant", VARIANTS)
@@ -240,6 +240,79 @@ def test_two_pair_cluster_multicast_variant(M, N, K):
     assert np.array_equal(y4, run("fused", 4, A, W1, W2))
 
 
+@pytest.mark.parametrize("M,N,K,div", [
+    (2560, 4864, 128, 0),   # 5 x 38 = 190 super tiles on 74 pairs: two full waves + a dense tail
+    (2560, 4864, 136, 2),   # ... the same tail forced into row-block units (K % 64 != 0)
+    (2305, 4872, 64, 4),    # ... and into row-block x 64-column units; ragged M and N
+    (1024, 5760, 200, 0),   # 90 tiles: 16 tail tiles -> the policy's quarter units
+    (1024, 6656, 64, 0),    # 104 tiles: 30 tail tiles -> row-block units
+    (768, 392, 1096, 0),    # second row tile has one block only (rows 512..767)
+    (769, 392, 328, 0),     # ... and a second block of a single row
+    (300, 136, 72, 0), (8, 128, 64, 0),
+])
+def test_super_tile_variant(M, N, K, div, swiglu_env):
+    """a3': the 512 x 128 super tile per CTA pair (two 128-row blocks per CTA share every weight
+    stage; all of TMEM is one tile; row blocks skewed at tile boundaries).  Many tiles per pair,
+    every cut of the last wave (none / row blocks / row blocks x column halves), every skew,
+    ragged M (a super tile with one block).  Same k order and MMA shapes as the 256-row pair
+    kernel, so the result is bit-identical to it."""
+    if div:
+        swiglu_env("SWIGLU_TAIL_KSPLIT", div)
+    A, W1, W2 = inputs.make_case(M, N, K, seed=490 + M + N + K, std=0.05)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+    y5 = run("fused", 5, A, W1, W2)
+    assert_parity(y5, y_ref, ("super tile", M, N, K, div))
+    for skew in (1, 2, 3):
+        swiglu_env("SWIGLU_SKEW", skew)
+        assert np.array_equal(run("fused", 5, A, W1, W2), y5), ("skew", skew)
+    swiglu_env("SWIGLU_SKEW", 4)
+    swiglu_env("SWIGLU_TAIL_KSPLIT", 0)
+    swiglu_env("SWIGLU_NO_TAIL_SPLIT", 1)
+    assert np.array_equal(run("fused", 5, A, W1, W2), y5), "uncut last wave"
+    assert np.array_equal(run("fused", 1, A, W1, W2), y5), "256-row pair kernel"
+
+
+@pytest.mark.parametrize("M,N,K,div", [(2560, 4864, 128, 0), (2305, 4872, 72, 2), (1024, 12032, 64, 0),
+                                       (768, 392, 328, 0)])
+def test_super_tile_gemm_of_the_unfused_path(M, N, K, div, swiglu_env):
+    """a7 with the super-tile GEMM (512 x 256 plain tiles, two row blocks per CTA): several waves,
+    cut and uncut last waves, one-block row tiles; bit-identical to the 256-row pair GEMM."""
+    if div:
+        swiglu_env("SWIGLU_TAIL_KSPLIT", div)
+    A, W1, W2 = inputs.make_case(M, N, K, seed=497 + M + N + K, std=0.05)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+    y3 = run("unfused", 3, A, W1, W2)
+    assert_parity(y3, y_ref, ("super-tile gemm", M, N, K, div))
+    assert np.array_equal(run("unfused", 1, A, W1, W2), y3)
+    dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+    B.swiglu_glu_mlp_layout(dev(A), dev(np.ascontiguousarray(W1.T)), dev(np.ascontiguousarray(W2.T)), dY,
+                            "silu", B.WEIGHTS_NK, unfused=True, variant=3)
+    torch.cuda.synchronize()
+    assert np.array_equal(host(dY), y3), "[N,K] weights"
+
+
+def test_super_tile_variant_other_operand_modes(swiglu_env):
+    """Prepacked weights and FP8 operands through the super-tile kernel, last wave cut into
+    quarter units (single-slab boxes / N = 128 instructions)."""
+    swiglu_env("SWIGLU_TAIL_KSPLIT", 4)
+    M, N, K = 2305, 4872, 256
+    A, W1, W2 = inputs.make_case(M, N, K, seed=495, std=0.05)
+    y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+    Wp = torch.empty(B.swiglu_packed_weight_bytes(N, K) // 2, dtype=torch.int16, device="cuda")
+    B.swiglu_pack_weights(dev(W1), dev(W2), Wp, N, K)
+    dY = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device="cuda")
+    B.swiglu_glu_mlp_packed(dev(A), Wp, dY, "silu", 5)
+    torch.cuda.synchronize()
+    assert_parity(host(dY), y_ref, "super tile, packed")
+    A8, W18, W28, sg, su = inputs.make_fp8_case(M, N, 512, seed=496, std=0.05)
+    y8, _ = oracle.swiglu_oracle_fp8(A8, W18, W28, sg, su)
+    dY.fill_(float("nan"))
+    B.swiglu_mlp_fp8(torch.from_numpy(A8).cuda(), torch.from_numpy(W18).cuda(),
+                     torch.from_numpy(W28).cuda(), dY, sg, su, 5)
+    torch.cuda.synchronize()
+    assert_parity(host(dY), y8, "super tile, fp8")
+
+
 def test_small_m_variant_rejects_large_m():
     A, W1, W2 = inputs.make_case(129, 128, 64, seed=1)
     with pytest.raises(B.SwigluError) as e:
@@ -333,7 +406,7 @@ ACTS = ["gelu", "gelu_tanh", "relu"]
 
 
 @pytest.mark.parametrize("act", ACTS)
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("M,N,K", [(16, 392, 328), (100, 1160, 200), (128, 4864, 896)])
 def test_other_gated_activations_every_fused_variant(act, variant, M, N, K):
     """GeGLU (erf and tanh forms) and ReGLU through every fused kernel, std chosen so Gate
@@ -394,7 +467,7 @@ def test_elementwise_stage_other_activations(act):
     assert_parity(host(dY), y_ref, ("act_mul", act))
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("M,N,K", [(1, 128, 64), (16, 392, 328), (100, 1160, 200), (128, 4864, 896),
                                    (7, 136, 72)])
 def test_nk_weight_layout_every_fused_variant(variant, M, N, K):
