@@ -517,7 +517,7 @@ def run_reference(args, ranks):
 # ---------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------
-def read_traffic(name, M):
+def read_traffic(name, M, kernel=None):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, copied
     from the committed `ncu --set full` captures (profiles/traffic.csv names the summary each
     row comes from), or (None, None) when that (workload, M) has not been captured."""
@@ -526,7 +526,8 @@ def read_traffic(name, M):
     try:
         hit = None
         for row in csv.DictReader(open(path)):
-            if row["workload"] == name and int(row["M"]) == int(M):
+            if row["workload"] == name and int(row["M"]) == int(M) and (
+                    kernel is None or row["kernel"] == kernel):
                 hit = row                                   # the last (newest) row wins
         if hit:
             return int(hit["dram_bytes_read"]) + int(hit["dram_bytes_write"]), hit["source"]
@@ -596,7 +597,8 @@ def run_ours(args, ranks):
         peak = peaks["bf16_tflops_sustained"] if long_run else peaks["bf16_tflops"]
     else:
         achieved, peak, runit = algo_bytes(Mdom, wl.N, wl.K) / (dom_ms * 1e-3) / 1e9, peaks["hbm_gbs"], "GB/s"
-    traffic, traffic_src = read_traffic(wl.name, Mdom)
+    traffic, traffic_src = read_traffic(
+        wl.name, Mdom, B.swiglu_variant_name(B.swiglu_selected_variant(Mdom, wl.N, wl.K)))
     roofline = {"bound": bound, "achieved": round(achieved, 2), "peak": peak, "unit": runit,
                 "frac": round(achieved / peak, 4), "traffic": traffic, "traffic_source": traffic_src,
                 "algorithmic_bytes": algo_bytes(Mdom, wl.N, wl.K),
