@@ -38,16 +38,25 @@ constexpr int kSmallPrefetchMax = 32;     // k-blocks per CTA prefetched to L2 (
 // kDeep: one CTA per SM with a six-stage ring (up to 204 KB of weights in flight per CTA) instead
 // of two co-resident CTAs with three stages each: half the CTAs (and clusters) to launch for the
 // same bytes in flight, used when n-tiles x S fits one CTA per SM (MP <= 32 only).
-template <int MP, bool kDeep = false>
+// kStack: a 64-column tile whose W1 slab and W2 slab are STACKED into one 128-row UMMA operand
+// (rows 0-63 = 64 columns of W1, rows 64-127 = the same 64 columns of W2): one MMA per k-step,
+// Gate^T in TMEM lanes 0-63 and Up^T in lanes 64-127 of the same MP columns.  Twice the tiles
+// of the 128-column form, so shapes with N/128 < #SMs (0.5B, 1.5B) fill the GPU WITHOUT a
+// cluster split of K: no cluster launch (an empty cluster-of-4 launch alone is 3.6 us in a
+// dependent chain against 1.7 us without clusters, profiles/r02_decode_study.md), no DSMEM
+// reduction, no cluster barriers.  One CTA per SM with a deep ring of 18 KB stages.
+template <int MP, bool kDeep = false, bool kStack = false>
 struct SmallCfg {
   static_assert(!kDeep || MP <= 32, "deep ring: MP <= 32");
+  static_assert(!kStack || (MP <= 32 && !kDeep), "stacked 64-column tile: MP <= 32, always a deep ring");
+  static constexpr int kTileN = kStack ? 64 : 128;  // output columns per tile
   static constexpr int kCtasPerSm = kDeep ? 1 : ((MP <= 64) ? 2 : 1);
-  static constexpr int kStages = kDeep ? 6 : ((MP <= 32) ? 3 : (MP == 64 ? 2 : 4));
-  static constexpr int kWBytes = 128 * BK * 2;  // one W tile: 128 n x 64 k = 16 KB
+  static constexpr int kStages = kStack ? 5 : kDeep ? 6 : ((MP <= 32) ? 3 : (MP == 64 ? 2 : 4));
+  static constexpr int kWBytes = kTileN * BK * 2;  // one W tile: 128 (64) n x 64 k = 16 (8) KB
   static constexpr int kABytes = MP * BK * 2;   // MP tokens x 64 k
   static constexpr int kStageBytes = 2 * kWBytes + kABytes;
-  static constexpr int kPartialBytes = 2 * MP * 128 * 4;  // fp32 Gate^T|Up^T, aliases the ring
-  static constexpr int kTmemCols = (2 * MP < 32) ? 32 : 2 * MP;
+  static constexpr int kPartialBytes = 2 * MP * kTileN * 4;  // fp32 Gate^T|Up^T, aliases the ring
+  static constexpr int kTmemCols = kStack ? 32 : ((2 * MP < 32) ? 32 : 2 * MP);
   static constexpr int kSmemBytes = kStages * kStageBytes + 256 + 1024;
   static_assert(kPartialBytes <= kStages * kStageBytes, "partials must fit in the ring");
 };
@@ -81,14 +90,15 @@ __device__ __forceinline__ float4 ld_dsmem_v4(uint32_t cluster_addr) {
 //   p.U = Up) instead of going through the activation -- one launch for both projections, the
 //   "merged gate_up_proj" serving stacks run before their silu_and_mul kernel.
 template <int MP, int kAct = kActSilu, int kWMode = kWeightsKN, bool kStoreGU = false,
-          bool kDeep = false>
-__global__ void __launch_bounds__(kSmallThreads, SmallCfg<MP, kDeep>::kCtasPerSm)
+          bool kDeep = false, bool kStack = false>
+__global__ void __launch_bounds__(kSmallThreads, SmallCfg<MP, kDeep, kStack>::kCtasPerSm)
 smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
                      const __grid_constant__ CUtensorMap tmap_w1,
                      const __grid_constant__ CUtensorMap tmap_w2, uint16_t* __restrict__ Y,
                      const SmallParams p) {
-  using Cfg = SmallCfg<MP, kDeep>;
+  using Cfg = SmallCfg<MP, kDeep, kStack>;
   constexpr int kStages = Cfg::kStages;
+  constexpr int kTileN = Cfg::kTileN;
   constexpr bool kF8 = (kWMode == kOperandsFp8);   // E4M3 A and [N,K] weights (gemm kernel header)
   constexpr bool kWK = (kWMode == kWeightsNK) || kF8;
   constexpr bool kPacked = (kWMode == kWeightsPacked);
@@ -109,7 +119,7 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   const int S = p.ksplit;
   const uint32_t rank = (S > 1) ? cluster_ctarank() : 0u;
   const int n_tile = blockIdx.x / S;
-  const int n_base = n_tile * 128;
+  const int n_base = n_tile * kTileN;
   const int k_blocks = (p.K + kBKe - 1) / kBKe;
   const int kb_begin = (int)(((long long)k_blocks * rank) / S);
   const int kb_end = (int)(((long long)k_blocks * (rank + 1)) / S);
@@ -120,7 +130,11 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     const uint32_t fb = full_bar(s);
     const int k0 = kb * kBKe;
     if constexpr (kPacked) {
-      tma_load_3d(smem_w(s), &tmap_w1, fb, 0, k0, n_tile * 4, kEvictFirst);  // g0 u0 g1 u1: 32 KB
+      // g0 u0 g1 u1: 32 KB (stacked 64-column tile: its g u pair, 16 KB)
+      tma_load_3d(smem_w(s), &tmap_w1, fb, 0, k0, n_tile * (kTileN / 32), kEvictFirst);
+    } else if constexpr (kStack) {
+      tma_load_2d(smem_w(s), &tmap_w1, fb, kWK ? k0 : n_base, kWK ? n_base : k0, kEvictFirst);
+      tma_load_2d(smem_w(s) + 8192, &tmap_w2, fb, kWK ? k0 : n_base, kWK ? n_base : k0, kEvictFirst);
     } else {
       // one 64-column x 64-k slab per load; inner tensor-map dimension is N ([K,N]) or K ([N,K])
       auto load_w = [&](uint32_t dst, const CUtensorMap* tm, int n) {
@@ -168,7 +182,7 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       // the rest of the CTA's weight stream: L2 prefetch, one k-block per lane
       const int kb = kb_begin + kStages + (int)lane;
       if (live && (int)lane < p.prefetch_blocks && kb < kb_end)
-        tma_prefetch_l2_3d(&tmap_w1, 0, kb * kBKe, n_tile * 4);
+        tma_prefetch_l2_3d(&tmap_w1, 0, kb * kBKe, n_tile * (kTileN / 32));
       if (lane == 0 && live) {
         pdl_wait_prior_grid();  // A may be the previous kernel's output
         SWIGLU_TRACE_POINT(2);
@@ -180,9 +194,9 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       if (live && (int)lane < p.prefetch_blocks && kb < kb_end) {
         const int k0 = kb * kBKe;
         tma_prefetch_l2_2d(&tmap_w1, kWK ? k0 : n_base, kWK ? n_base : k0);
-        tma_prefetch_l2_2d(&tmap_w1, kWK ? k0 : n_base + 64, kWK ? n_base + 64 : k0);
+        if (!kStack) tma_prefetch_l2_2d(&tmap_w1, kWK ? k0 : n_base + 64, kWK ? n_base + 64 : k0);
         tma_prefetch_l2_2d(&tmap_w2, kWK ? k0 : n_base, kWK ? n_base : k0);
-        tma_prefetch_l2_2d(&tmap_w2, kWK ? k0 : n_base + 64, kWK ? n_base + 64 : k0);
+        if (!kStack) tma_prefetch_l2_2d(&tmap_w2, kWK ? k0 : n_base + 64, kWK ? n_base + 64 : k0);
       }
       if (lane == 0 && live) {
         // W or A may be the previous kernel's output: real loads only after the grid dependency
@@ -236,6 +250,16 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           // step, the two 64-column atoms 8 KB apart (Gate at +0, Up at +16 KB).  Packed: the
           // atoms g0, g1 are 16 KB apart (u0 sits between them), Up starts at +8 KB.
           // [N,K] weights: K-major, +32 B per step, the two 64-row slabs are contiguous.
+          if constexpr (kStack) {
+            // stacked operand: rows 0-63 = the W1 slab, rows 64-127 = the W2 slab 8 KB behind it
+            // (MN-major: the second 64-element atom; K-major: the next 64 rows)
+            const uint64_t wd = kWK ? smem_desc_sw128(sw + k * (UMMA_K * 2), 16, 1024)
+                                    : smem_desc_sw128(sw + k * (UMMA_K * 128), 8192, 1024);
+            const uint64_t ad = smem_desc_sw128(smem_act(s) + k * (UMMA_K * 2), 16, 1024);
+            if constexpr (kF8) umma_f8<1>(tmem_base, wd, ad, idesc, acc);
+            else umma_bf16<1>(tmem_base, wd, ad, idesc, acc);  // lanes 0-63 Gate^T, 64-127 Up^T
+            continue;
+          }
           uint64_t w1d, w2d;
           if constexpr (kWK) {
             w1d = smem_desc_sw128(sw + k * (UMMA_K * 2), 16, 1024);
@@ -281,6 +305,22 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       for (int c = 0; c < MP / 16; ++c) {
         if (c * 16 >= p.M) break;  // rows >= M are never read back
         uint32_t g[16], u[16];
+        if constexpr (kStack) {
+          // lanes 0-63 hold Gate^T, lanes 64-127 Up^T of columns n = nl % 64
+          if (have) {
+            tmem_ld_32x32b_x16(tacc + c * 16, g);
+            tmem_ld_wait();
+          } else {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) g[j] = 0u;
+          }
+          const uint32_t row0 = (q >> 1) * MP + c * 16, col = nl & 63u;
+#pragma unroll
+          for (int j = 0; j < 16; ++j)
+            asm volatile("st.shared.b32 [%0], %1;" ::"r"(part + ((row0 + j) * 64u + col) * 4u), "r"(g[j])
+                         : "memory");
+          continue;
+        }
         if (have) {
           tmem_ld_32x32b_x16(tacc + c * 16, g);
           tmem_ld_32x32b_x16(tacc + MP + c * 16, u);
@@ -313,8 +353,9 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     if (warp >= 2) {
       pdl_wait_prior_grid();  // Y may still be being written by the previous kernel in the stream
       const uint32_t et = threadIdx.x - 64u;
-      const uint32_t c4 = (et & 31u) * 4u;  // 4 consecutive output columns per thread
-      const uint32_t sub = et >> 5;         // 4 row slots
+      constexpr uint32_t kColThreads = kTileN / 4, kRowSlots = 128 / kColThreads;
+      const uint32_t c4 = (et % kColThreads) * 4u;  // 4 consecutive output columns per thread
+      const uint32_t sub = et / kColThreads;        // 4 (stacked tile: 8) row slots
       const int n = n_base + (int)c4;
       uint32_t peer[8];
 #pragma unroll
@@ -338,18 +379,18 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
         }
       };
       auto add4 = [](float4& a, const float4& b) { a.x += b.x; a.y += b.y; a.z += b.z; a.w += b.w; };
-      for (int m0 = (int)rank + S * (int)sub; m0 < p.M; m0 += 8 * S) {
-        const int m1 = m0 + 4 * S;
+      for (int m0 = (int)rank + S * (int)sub; m0 < p.M; m0 += 2 * (int)kRowSlots * S) {
+        const int m1 = m0 + (int)kRowSlots * S;
         const bool two = m1 < p.M;
         float4 g0[8], u0[8], g1[8], u1[8];
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
           if (r < S) {
-            g0[r] = ld_dsmem_v4(peer[r] + (uint32_t)(m0 * 128 + (int)c4) * 4u);
-            u0[r] = ld_dsmem_v4(peer[r] + (uint32_t)((MP + m0) * 128 + (int)c4) * 4u);
+            g0[r] = ld_dsmem_v4(peer[r] + (uint32_t)(m0 * kTileN + (int)c4) * 4u);
+            u0[r] = ld_dsmem_v4(peer[r] + (uint32_t)((MP + m0) * kTileN + (int)c4) * 4u);
             if (two) {
-              g1[r] = ld_dsmem_v4(peer[r] + (uint32_t)(m1 * 128 + (int)c4) * 4u);
-              u1[r] = ld_dsmem_v4(peer[r] + (uint32_t)((MP + m1) * 128 + (int)c4) * 4u);
+              g1[r] = ld_dsmem_v4(peer[r] + (uint32_t)(m1 * kTileN + (int)c4) * 4u);
+              u1[r] = ld_dsmem_v4(peer[r] + (uint32_t)((MP + m1) * kTileN + (int)c4) * 4u);
             }
           }
         }

@@ -90,6 +90,7 @@ struct Env {
   bool no_pdl = false, no_prefetch = false, no_early = false, no_tail_split = false,
        no_tail_ksplit = false, no_w_evict_first = false, no_tmap_cache = false;
   int smallm_deep = -1;  // -1 automatic, 0 never, 1 whenever it fits
+  int smallm_stack = -1;  // stacked 64-column decode tile: -1 automatic, 0 never, 1 whenever instantiated
   int w_policy = -1, a_policy = -1;  // large-M kernel L2 hints: -1 automatic, 0 normal, 1 first, 2 last
 };
 Env g_env;
@@ -113,6 +114,7 @@ void load_env() {
   e.no_tmap_cache = env_int("SWIGLU_NO_TMAP_CACHE", 0) != 0;
   e.smallm_deep = env_int("SWIGLU_SMALLM_DEEP", -1);
   e.skew = env_int("SWIGLU_SKEW", 4);
+  e.smallm_stack = env_int("SWIGLU_SMALLM_STACK", -1);
   e.w_policy = env_int("SWIGLU_W_POLICY", -1);
   e.a_policy = env_int("SWIGLU_A_POLICY", -1);
   g_env = e;
@@ -266,11 +268,15 @@ int set_smem_attrs() {
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kAct, kWK>, attr, SmallCfg<32>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kAct, kWK>, attr, SmallCfg<64>::kSmemBytes));
   CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<128, kAct, kWK>, attr, SmallCfg<128>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kAct, kWK, false, false, true>, attr, SmallCfg<16, false, true>::kSmemBytes));
+  CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kAct, kWK, false, false, true>, attr, SmallCfg<32, false, true>::kSmemBytes));
   if constexpr (kWK == kWeightsKN || kWK == kWeightsPacked) {
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kAct, kWK, false, true>, attr, SmallCfg<16, true>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kAct, kWK, false, true>, attr, SmallCfg<32, true>::kSmemBytes));
   }
   if constexpr (kAct == kActSilu && kWK != kWeightsPacked && kWK != kOperandsFp8) {  // plain GEMMs: no activation
+    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kActSilu, kWK, true, false, true>, attr, SmallCfg<16, false, true>::kSmemBytes));
+    CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kActSilu, kWK, true, false, true>, attr, SmallCfg<32, false, true>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<16, kActSilu, kWK, true>, attr, SmallCfg<16>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<32, kActSilu, kWK, true>, attr, SmallCfg<32>::kSmemBytes));
     CUDA_TRY(cudaFuncSetAttribute(smallm_swiglu_kernel<64, kActSilu, kWK, true>, attr, SmallCfg<64>::kSmemBytes));
@@ -613,14 +619,27 @@ int smallm_ksplit(int sm_count, int ctas_per_sm, int mp, int64_t n_tiles, int64_
   return (int)s;
 }
 
-template <int MP, int kAct, int kWMode, bool kStoreGU = false, bool kDeep = false>
+template <int MP, int kAct, int kWMode, bool kStoreGU = false, bool kDeep = false, bool kStack = false>
 int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const void* W2,
                      void* Y, void* U, int64_t M, int64_t N, int64_t K, cudaStream_t stream,
                      int probe = 0, float scale_gate = 1.0f, float scale_up = 1.0f) {
   using namespace swiglu;
+  // Stacked 64-column tile (one CTA per SM, no cluster): when the 128-column tiles cannot fill
+  // the GPU but the 64-column ones fit one wave -- 0.5B and 1.5B-class N -- the GPU fills without
+  // a cluster split of K.
+  if constexpr (!kStack && !kDeep && MP <= 32) {
+    const int64_t nt128 = (N + 127) / 128, nt64 = (N + 63) / 64;
+    // (not for prepacked weights: there the 128-column forms already send every weight load ahead
+    // of the grid dependency and measure faster -- 1.5B M=16: 10.9 vs 12.2 us, 0.5B: 6.1 vs 6.6)
+    const bool automatic = env().smallm_stack < 0 && nt128 < d.sm_count && nt64 <= 2 * d.sm_count &&
+                           env().smallm_deep < 0 && kWMode != kWeightsPacked;
+    if (env().smallm_stack == 1 || automatic)
+      return launch_smallm_mp<MP, kAct, kWMode, kStoreGU, false, true>(d, A, W1, W2, Y, U, M, N, K, stream,
+                                                                       probe, scale_gate, scale_up);
+  }
   // Deep-ring form (one CTA per SM, six stages): taken when it is instantiated for this
   // (MP, weights) and some S <= 4 puts n-tiles x S on at most one CTA per SM.
-  if constexpr (!kDeep && !kStoreGU && MP <= 32 && (kWMode == kWeightsKN || kWMode == kWeightsPacked)) {
+  if constexpr (!kStack && !kDeep && !kStoreGU && MP <= 32 && (kWMode == kWeightsKN || kWMode == kWeightsPacked)) {
     const int64_t nt = (N + 127) / 128;
     const bool fits = nt < d.sm_count && (env().ksplit <= 0 || nt * env().ksplit <= d.sm_count);
     // automatic: only with prepacked (constant) weights and when the CTA's whole K-range fits the
@@ -646,16 +665,28 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   }
   if constexpr (kWMode == kOperandsFp8) {
   } else if constexpr (kWMode == kWeightsPacked) {
-    if ((rc = make_tmap_packed(&tw1, W1, K, packed_slabs(N), 4))) return rc;  // W1 = Wp
+    if ((rc = make_tmap_packed(&tw1, W1, K, packed_slabs(N), kStack ? 2 : 4))) return rc;  // W1 = Wp
     tw2 = tw1;
   } else {
     if ((rc = make_tmap(&tw1, W1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
     if ((rc = make_tmap(&tw2, W2, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
   }
-  const int64_t n_tiles = (N + 127) / 128, k_blocks = (K + kBKe - 1) / kBKe;
+  using Cfg = SmallCfg<MP, kDeep, kStack>;
+  const int64_t n_tiles = (N + Cfg::kTileN - 1) / Cfg::kTileN, k_blocks = (K + kBKe - 1) / kBKe;
   SmallParams p;
   p.M = (int)M; p.N = (int)N; p.K = (int)K;
-  p.ksplit = smallm_ksplit(d.sm_count, SmallCfg<MP, kDeep>::kCtasPerSm, MP, n_tiles, k_blocks);
+  p.ksplit = smallm_ksplit(d.sm_count, Cfg::kCtasPerSm, MP, n_tiles, k_blocks);
+  if constexpr (kStack) {
+    // stacked tile: a cluster only when the 64-column tiles alone leave half the SMs idle
+    // (0.5B: 76 tiles -> S = 2; 1.5B: 140 tiles -> S = 1, measured 11.5 vs 12.4 us at M = 16)
+    int64_t s = (d.sm_count + n_tiles / 2) / n_tiles;
+    if (s > 4) s = 4;
+    while (s > 1 && k_blocks / s < 4) --s;
+    if (s < 1) s = 1;
+    if (env().ksplit > 0) s = env().ksplit > 8 ? 8 : env().ksplit;
+    if (s > k_blocks) s = k_blocks;
+    p.ksplit = (int)s;
+  }
   p.ldy = N;
   p.U = (uint16_t*)U;
   p.probe = probe;
@@ -664,7 +695,7 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   p.clk = g_clk.load(std::memory_order_relaxed);
   // L2 prefetch ahead of the grid dependency: at most ~32 MiB over the whole grid
   const int64_t grid = n_tiles * p.ksplit;
-  int64_t pf = (32ll << 20) / (grid * 2 * SmallCfg<MP, kDeep>::kWBytes);
+  int64_t pf = (32ll << 20) / (grid * 2 * Cfg::kWBytes);
   if (pf > kSmallPrefetchMax) pf = kSmallPrefetchMax;
   if (env().no_prefetch) pf = 0;
   p.prefetch_blocks = (int)pf;
@@ -675,7 +706,7 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   memset(&cfg, 0, sizeof cfg);
   cfg.gridDim = dim3((unsigned)(n_tiles * p.ksplit));
   cfg.blockDim = dim3(kSmallThreads);
-  cfg.dynamicSmemBytes = SmallCfg<MP, kDeep>::kSmemBytes;
+  cfg.dynamicSmemBytes = Cfg::kSmemBytes;
   cfg.stream = stream;
   cudaLaunchAttribute attrs[2];
   int na = 0;
@@ -693,7 +724,7 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   }
   cfg.attrs = attrs;
   cfg.numAttrs = na;
-  CUDA_TRY(cudaLaunchKernelEx(&cfg, smallm_swiglu_kernel<MP, kAct, kWMode, kStoreGU, kDeep>, ta, tw1,
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, smallm_swiglu_kernel<MP, kAct, kWMode, kStoreGU, kDeep, kStack>, ta, tw1,
                               tw2, (uint16_t*)Y, p));
   return SWIGLU_OK;
 }

@@ -103,10 +103,24 @@ def test_large_m_kernels_on_odd_shapes(kind, variant, M, N, K):
                                    (64, 4864, 896), (5, 29568, 512), (65, 264, 200),
                                    (100, 1160, 328), (128, 4864, 896), (127, 8960, 1536),
                                    (128, 128, 64), (3, 8, 8), (48, 136, 8)])
-def test_small_m_kernel_on_odd_shapes(M, N, K):
+def test_small_m_kernel_on_odd_shapes(M, N, K, swiglu_env):
+    """a6 in both tile forms: the 128-column tile (cluster split of K where that fills the GPU) and,
+    for M <= 32, the stacked 64-column tile (W1 slab | W2 slab as one 128-row operand, no cluster).
+    Both accumulate every output in the same k order: bit-identical when K is not split."""
     A, W1, W2 = inputs.make_case(M, N, K, seed=200 + M + N + K, std=0.05)
     y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
     assert_parity(run("fused", 2, A, W1, W2), y_ref, ("smallm", M, N, K))
+    swiglu_env("SWIGLU_SMALLM_STACK", 0)
+    swiglu_env("SWIGLU_KSPLIT", 1)
+    y128 = run("fused", 2, A, W1, W2)
+    assert_parity(y128, y_ref, ("smallm 128-column tile", M, N, K))
+    swiglu_env("SWIGLU_SMALLM_STACK", 1)
+    y64 = run("fused", 2, A, W1, W2)
+    assert_parity(y64, y_ref, ("smallm stacked 64-column tile", M, N, K))
+    assert np.array_equal(y64, y128)
+    assert_parity(run("unfused", 2, A, W1, W2), y_ref, ("merged Gate|Up GEMM, stacked tile", M, N, K))
+    swiglu_env("SWIGLU_KSPLIT", 3)   # the stacked tile under a forced cluster split of K
+    assert_parity(run("fused", 2, A, W1, W2), y_ref, ("smallm stacked, S=3", M, N, K))
 
 
 @pytest.mark.parametrize("ksplit", [1, 2, 3, 5, 8])
