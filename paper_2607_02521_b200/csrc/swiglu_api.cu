@@ -85,7 +85,7 @@ int env_int(const char* name, int dflt) {
 // first call into the library (and again only on swiglu_reload_env()): the hot path does no
 // getenv.  All default to "off" / "automatic".
 struct Env {
-  int variant = -1, unfused_variant = -1, ksplit = 0, group_m = 0, host_chunks = 4, tail_ksplit = 0;
+  int variant = -1, unfused_variant = -1, ksplit = 0, group_m = 0, host_chunks = 8, tail_ksplit = 0;
   int skew = 4;  // super-tile kernel: k-blocks row block 0 leads block 1 at tile boundaries
   bool no_pdl = false, no_prefetch = false, no_early = false, no_tail_split = false,
        no_tail_ksplit = false, no_w_evict_first = false, no_tmap_cache = false;
@@ -103,8 +103,8 @@ void load_env() {
   e.group_m = env_int("SWIGLU_GROUP_M", 0);
   e.tail_ksplit = env_int("SWIGLU_TAIL_KSPLIT", 0);
   if (e.tail_ksplit > 8) e.tail_ksplit = 8;
-  e.host_chunks = env_int("SWIGLU_HOST_CHUNKS", 4);
-  if (e.host_chunks <= 0) e.host_chunks = 4;
+  e.host_chunks = env_int("SWIGLU_HOST_CHUNKS", 8);
+  if (e.host_chunks <= 0) e.host_chunks = 8;
   e.no_pdl = env_int("SWIGLU_NO_PDL", 0) != 0;
   e.no_prefetch = env_int("SWIGLU_NO_PREFETCH", 0) != 0;
   e.no_early = env_int("SWIGLU_NO_EARLY", 0) != 0;
