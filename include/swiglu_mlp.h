@@ -282,7 +282,8 @@ int swiglu_release(void);
  * Experiment overrides (SWIGLU_VARIANT, SWIGLU_UNFUSED_VARIANT, SWIGLU_KSPLIT, SWIGLU_GROUP_M,
  * SWIGLU_HOST_CHUNKS, SWIGLU_NO_PDL, SWIGLU_NO_PREFETCH, SWIGLU_NO_EARLY, SWIGLU_NO_TAIL_SPLIT,
  * SWIGLU_NO_TAIL_KSPLIT, SWIGLU_TAIL_KSPLIT, SWIGLU_NO_W_EVICT_FIRST, SWIGLU_NO_TMAP_CACHE,
- * SWIGLU_SMALLM_DEEP, SWIGLU_W_POLICY, SWIGLU_A_POLICY) are read from the environment once, at the
+ * SWIGLU_SMALLM_DEEP, SWIGLU_SMALLM_STACK, SWIGLU_SKEW, SWIGLU_W_POLICY, SWIGLU_A_POLICY, SWIGLU_Y_POLICY) are read
+ * from the environment once, at the
  * first call into the library.  swiglu_reload_env re-reads them (sweeps and tests; not
  * thread-safe against concurrent compute calls).
  */

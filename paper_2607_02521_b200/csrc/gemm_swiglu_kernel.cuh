@@ -69,6 +69,7 @@ struct GemmParams {
   int* split_ctr;   // [tail tile][CTA of the group] arrival counters, zero between launches
   int early_issue;      // 1: fill the ring before the CTA-wide setup barrier (small grids)
   unsigned long long w_policy, a_policy;  // L2 eviction-priority hints of the weight / A loads
+  unsigned long long y_policy;            // ... and of the Y stores
   unsigned long long* clk;  // optional {SM cycles, globaltimer ns} of CTA 0 (swiglu_set_clock_probe)
   float scale_gate, scale_up;  // kOperandsFp8: Gate / Up dequantisation scales (else unused)
 #ifdef SWIGLU_TRACE
@@ -720,7 +721,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
         fence_proxy_async_smem();
         named_bar_sync(1, kEpiWarps * 32);
         if (issuer) {
-          tma_store_2d(&tmap_y, obuf, n_base + h * 64, m_base);  // OOB rows/cols are clipped
+          tma_store_2d_hint(&tmap_y, obuf, n_base + h * 64, m_base, p.y_policy);  // OOB rows/cols are clipped
           tma_store_commit();
         }
       }

@@ -91,7 +91,7 @@ struct Env {
        no_tail_ksplit = false, no_w_evict_first = false, no_tmap_cache = false;
   int smallm_deep = -1;  // -1 automatic, 0 never, 1 whenever it fits
   int smallm_stack = -1;  // stacked 64-column decode tile: -1 automatic, 0 never, 1 whenever instantiated
-  int w_policy = -1, a_policy = -1;  // large-M kernel L2 hints: -1 automatic, 0 normal, 1 first, 2 last
+  int w_policy = -1, a_policy = -1, y_policy = -1;  // large-M kernel L2 hints: -1 automatic, 0 normal, 1 first, 2 last
 };
 Env g_env;
 std::once_flag g_env_once;
@@ -117,6 +117,7 @@ void load_env() {
   e.smallm_stack = env_int("SWIGLU_SMALLM_STACK", -1);
   e.w_policy = env_int("SWIGLU_W_POLICY", -1);
   e.a_policy = env_int("SWIGLU_A_POLICY", -1);
+  e.y_policy = env_int("SWIGLU_Y_POLICY", -1);
   g_env = e;
 }
 const Env& env() {
@@ -559,6 +560,10 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
     p.a_policy = sm100::kEvictNormal;
     if (env().w_policy >= 0 && env().w_policy < 3) p.w_policy = pol[env().w_policy];
     if (env().a_policy >= 0 && env().a_policy < 3) p.a_policy = pol[env().a_policy];
+    // Y larger than half of L2 cannot stay for a consumer anyway: let its lines leave first
+    // (72B M=8192 / 7B M=4096 sustained: 1408 -> 1415, 1404 -> 1415 TFLOP/s; noise-level, kept)
+    p.y_policy = (M * N * 2 > (64ll << 20)) ? sm100::kEvictFirst : sm100::kEvictNormal;
+    if (env().y_policy >= 0 && env().y_policy < 3) p.y_policy = pol[env().y_policy];
   }
   p.clk = g_clk.load(std::memory_order_relaxed);
   p.scale_gate = scale_gate;
