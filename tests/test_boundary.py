@@ -46,6 +46,27 @@ def test_version_status_strings_and_variant_table(lib):
     assert B.swiglu_launches_per_call(0, 4864, 896) == 0
 
 
+def test_large_m_dispatch_table(lib):
+    """Host-only table (no CUDA call): the 512-row super tile for M > 512 with K >= 2048 where its
+    wave efficiency is within 3 points of the 256-row pair kernel's, the pair kernel otherwise
+    (profiles/r02b_variant_sweep_super_tile.md); same rule for the unfused GEMM."""
+    name = lambda M, N, K, unfused=False: B.swiglu_variant_name(
+        B.swiglu_selected_variant(M, N, K, unfused=unfused), unfused=unfused)
+    for K, N in ((3584, 18944), (5120, 27648), (8192, 29568), (5120, 13824)):
+        for M in (1024, 2048, 4096, 8192):
+            assert "512x128" in name(M, N, K), (M, N, K)
+            assert "512x256" in name(M, N, K, unfused=True), (M, N, K)
+        for M in (129, 256, 512):
+            assert name(M, N, K) == "fused_2cta_256x128", (M, N, K)
+    for K, N in ((896, 4864), (1536, 8960)):            # short K: the skewed tile boundary does not amortise
+        for M in (256, 1024, 4096, 8192):
+            assert name(M, N, K) == "fused_2cta_256x128", (M, N, K)
+            assert "256x256" in name(M, N, K, unfused=True), (M, N, K)
+    # no workspace for the super tile (its last wave is cut into row-block / quarter units, not in K)
+    assert B.swiglu_workspace_bytes(8192, 29568, 8192, unfused=False) == 0
+    assert B.swiglu_workspace_bytes(512, 29568, 8192, unfused=False) > 0     # pair kernel, K-split tail
+
+
 def test_activation_table(lib):
     assert [B.swiglu_activation_name(i) for i in range(5)] == ["silu", "gelu", "gelu_tanh", "relu", None]
     assert B.ACTIVATIONS == {"silu": 0, "gelu": 1, "gelu_tanh": 2, "relu": 3}
