@@ -36,6 +36,7 @@ constexpr int UMMA_K = 16;   // k per tcgen05.mma (kind::f16)
 constexpr int kEpiWarps = 8;
 constexpr int kGemmThreads = 64 + 32 * kEpiWarps;  // warp 0 TMA, warp 1 MMA, warps 2-9 epilogue
 constexpr int kOutBufBytes = BM * 64 * 2;          // one 64-column bf16 output chunk (16 KB)
+constexpr int kQuarterBufBytes = 32 * 64 * 2;      // ... of which each TMEM lane quarter stages 32 rows (4 KB)
 
 // kUmmaN = accumulator columns per tile: 256 (fused: Gate 128 | Up 128; unfused: 256 plain
 // columns) or, for the narrow fused tile used when N/128 tiles cannot fill the GPU,
@@ -78,6 +79,12 @@ struct GemmParams {
 };
 
 // Debug-build timeline stamps (compiled out unless -DSWIGLU_TRACE): slot i of this CTA.
+// Per tile (8 slots): MMA thread 0-2 (+5, 6 in the super-tile kernel), epilogue 3, 4 (7: second
+// region); in the 256-row kernels slots 5-7 time chunk SWIGLU_TRACE_H of the epilogue (after the
+// first barrier / the TMEM loads / the second barrier).
+#ifndef SWIGLU_TRACE_H
+#define SWIGLU_TRACE_H 0
+#endif
 constexpr int kGemmTraceStride = 8 + 8 * 32;
 #ifdef SWIGLU_TRACE
 #define SWIGLU_TRACE_POINT(i)                                                         \
@@ -106,12 +113,25 @@ __device__ __forceinline__ void decode_tile(const GemmParams& p, int t, int& tm,
   tm = m0 + (r - tn * gm);
 }
 
+// 1 / x for 1 <= x <= 2^126 on the FMA pipe: exponent-flip seed (|error| <= 5 %) and two Newton
+// steps, relative error <= 7e-6 (fp32 arithmetic; the bf16 result keeps 8 bits).  The epilogue of
+// a tile is MUFU-bound (16 lanes per clock per SM against 128 FMA lanes): taking the reciprocal off
+// the MUFU pipe halves its MUFU work.
+__device__ __forceinline__ float rcp_ge1_fma(float x) {
+  float r = __int_as_float(0x7EF31000 - __float_as_int(x));
+  r = r * fmaf(-x, r, 2.0f);
+  return r * fmaf(-x, r, 2.0f);
+}
+// sigma(z) * p = p / (1 + 2^(-z*log2 e)), one MUFU (ex2).  The exponent is capped at 126 so that
+// 1 + e stays finite for any z (the result is then ~1e-38 * p: zero for every purpose here).
+__device__ __forceinline__ float sigmoid_mul(float z, float p) {
+  float e;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(fminf(z * -1.4426950408889634f, 126.0f)));
+  return p * rcp_ge1_fma(1.0f + e);
+}
 __device__ __forceinline__ float silu_mul(float g, float u) {
   // SiLU(g)*u = g*u / (1 + 2^(-g*log2 e)); fp32 throughout.
-  float e, r;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(g * -1.4426950408889634f));
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
-  return (g * u) * r;
+  return sigmoid_mul(g, g * u);
 }
 
 // Tile t of the schedule -> (row tile, first output column, width in output columns).
@@ -196,10 +216,7 @@ __device__ __forceinline__ float glu_mul(float g, float u) {
     // 0.5 g (1 + tanh(c (g + 0.044715 g^3))) = g * sigma(2c (g + 0.044715 g^3)): the SiLU
     // form with a cubic argument -- no cancellation in the negative tail.
     const float z = g * fmaf(0.07135481627f, g * g, 1.5957691216f);  // 2c*0.044715, 2c
-    float e, r;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(z * -1.4426950408889634f));
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
-    return (g * u) * r;
+    return sigmoid_mul(z, g * u);
   } else if constexpr (kAct == kActGelu) {
     // g * Phi(g), Phi(g) = erfc(-g / sqrt 2) / 2.  erfc(t), t >= 0, from Abramowitz & Stegun
     // 7.1.26: (a1 k + ... + a5 k^5) exp(-t^2), k = 1 / (1 + 0.3275911 t), |error| <= 1.5e-7 --
@@ -473,7 +490,9 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       uint32_t ph0 = 0;
       uint32_t it0 = 0, it1 = 0;  // uses of accumulator region 0 / 1 so far (barrier phases)
       const int L = min(max(p.skew, 1), kStages);
+      [[maybe_unused]] int it = -1;  // tile counter of the debug-build timeline stamps
       for (int t = group_id; t < total_tiles; t += num_groups) {
+        ++it;
         const TileUnit u = decode_unit<kOutCols, kMB>(p, t, k_blocks);
         const int n = u.kb1 - u.kb0;
         const uint32_t idesc = (u.w == 64) ? idesc_half : idesc_full;
@@ -523,19 +542,24 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           if (++s1 == kStages) s1 = 0;
         };
         mbar_wait(acc_empty_bar(0), aph0 ^ 1u);  // region 0 drained
+        SWIGLU_GEMM_TRACE(8 + it * 8 + 0);
         tcgen05_fence_after();
         for (int i = 0; i < H; ++i) do0();
+        SWIGLU_GEMM_TRACE(8 + it * 8 + 1);
         if (T == 0) umma_commit<kCtaGroup>(acc_full_bar(0), pair_mask);  // the whole K range fitted the head
         mbar_wait(acc_empty_bar(1), aph1 ^ 1u);  // region 1 drained
+        SWIGLU_GEMM_TRACE(8 + it * 8 + 2);
         tcgen05_fence_after();
         for (int i = 0; i < H; ++i) do1();
         for (int i = n - H - T; i > 0; --i) { do0(); do1(); }
         if (T > 0) {
           for (int i = 0; i < T; ++i) do0();
           umma_commit<kCtaGroup>(acc_full_bar(0), pair_mask);  // region 0 complete: drains under block 1's tail
+          SWIGLU_GEMM_TRACE(8 + it * 8 + 5);
           for (int i = 0; i < T; ++i) do1();
         }
         umma_commit<kCtaGroup>(acc_full_bar(1), pair_mask);
+        SWIGLU_GEMM_TRACE(8 + it * 8 + 6);
       }
     } else {
     int s = 0;
@@ -579,7 +603,8 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     const uint32_t q = warp & 3u;  // TMEM lane quarter this warp may read
     const uint32_t row = q * 32u + lane;
     const uint32_t eg = (warp - 2u) >> 2;  // 0: columns [0,32) of each 64-column chunk, 1: [32,64)
-    const bool issuer = (threadIdx.x == 64);
+    const bool issuer = (threadIdx.x == 64);         // K-split ticket, debug stamps
+    const bool q_issuer = (eg == 0u && lane == 0u);  // TMA stores of this lane quarter
     const uint32_t leader_acc_empty0 =
         (kCtaGroup == 2) ? mapa_shared(acc_empty_bar(0), crank & ~1u) : 0u;  // the pair leader's
     int it = 0;
@@ -597,7 +622,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       const uint32_t aph = (kMB == 2) ? ((reg_phase >> mb) & 1u) : ((it >> 1) & 1u);
       reg_phase ^= 1u << mb;
       mbar_wait(acc_full_bar(as), aph);
-      if (issuer) SWIGLU_GEMM_TRACE(8 + it * 8 + 3);
+      if (issuer) SWIGLU_GEMM_TRACE(8 + it * 8 + (mb == 0 ? 3 : 7));
       tcgen05_fence_after();
       const uint32_t tacc = tmem_base + ((q * 32u) << 16) + as * UMMA_N;
       // K-range unit of a tail tile: park the fp32 partial accumulators in the workspace
@@ -623,9 +648,9 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           }
           tcgen05_fence_before();
           __syncwarp();
-          if (lane == 0) {  // TMEM stage drained
-            if constexpr (kCtaGroup == 2) mbar_arrive_cluster(leader_acc_empty0 + 8u * as);
-            else mbar_arrive(acc_empty_bar(as));
+          if (lane == 0) {  // TMEM stage drained (relaxed: see the hand-back in the chunk loop)
+            if constexpr (kCtaGroup == 2) mbar_arrive_relaxed_cluster(leader_acc_empty0 + 8u * as);
+            else mbar_arrive_relaxed(acc_empty_bar(as));
           }
           __threadfence();  // partials visible device-wide before the arrival is counted
           named_bar_sync(1, kEpiWarps * 32);
@@ -644,10 +669,16 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       }
 #pragma unroll 1
       for (int h = 0; h < chunks; ++h, ++chunk_ctr) {
-        const uint32_t obuf = smem_out + (chunk_ctr & 1u) * kOutBufBytes;
+        // Each TMEM lane quarter is its own store pipeline: the two warps of quarter q (columns
+        // [0,32) and [32,64) of the chunk) share a double-buffered 32-row x 128-byte staging area,
+        // synchronise with each other only (named barrier 2 + q, 64 threads) and one of them issues
+        // the 64-column x 32-row TMA store.  The four quarters drift freely, so one quarter's TMEM
+        // loads and MUFU work overlap another's barrier and store issue.
+        const uint32_t obuf = smem_out + q * (2u * kQuarterBufBytes) + (chunk_ctr & 1u) * kQuarterBufBytes;
         // the TMA store that last read this buffer (2 chunks ago) must have finished reading
-        if (issuer) tma_store_wait_read<1>();
-        named_bar_sync(1, kEpiWarps * 32);
+        if (q_issuer) tma_store_wait_read<1>();
+        named_bar_sync(2u + q, 64);
+        if (issuer && kMB == 1 && h == SWIGLU_TRACE_H) SWIGLU_GEMM_TRACE(8 + it * 8 + 5);
         {
           const int c = (int)eg;  // this warp's half of the chunk
           uint32_t packed[16];
@@ -682,6 +713,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
               tmem_ld_32x32b_x32(tacc + gcol, g);
               tmem_ld_32x32b_x32(tacc + ucol, u);
               tmem_ld_wait();
+              if (issuer && kMB == 1 && h == SWIGLU_TRACE_H) SWIGLU_GEMM_TRACE(8 + it * 8 + 6);
             }
 #pragma unroll
             for (int j = 0; j < 16; ++j) {
@@ -706,29 +738,35 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
             tcgen05_fence_before();
             __syncwarp();
             if (lane == 0) {
-              if constexpr (kCtaGroup == 2) mbar_arrive_cluster(leader_acc_empty0 + 8u * as);
-              else mbar_arrive(acc_empty_bar(as));
+              // RELAXED arrive: the only thing the MMA thread needs from this warp is that its
+              // TMEM reads are over, and tcgen05.wait::ld above has already retired them into
+              // registers; there is no memory to publish.  (A release at cluster scope here cost
+              // 1.2 us per hand-back -- it drains this thread's earlier stores first: measured
+              // 3.4 -> 2.2 us per 128x128 tile epilogue.)
+              if constexpr (kCtaGroup == 2) mbar_arrive_relaxed_cluster(leader_acc_empty0 + 8u * as);
+              else mbar_arrive_relaxed(acc_empty_bar(as));
             }
           }
           // 128-byte swizzled staging: row r, 16-byte chunk j -> chunk (j ^ (r & 7))
 #pragma unroll
           for (int j = 0; j < 4; ++j) {
             const uint32_t chunk = (uint32_t)(c * 4 + j) ^ (row & 7u);
-            st_shared_v4(obuf + row * 128u + chunk * 16u, packed[4 * j], packed[4 * j + 1],
+            st_shared_v4(obuf + lane * 128u + chunk * 16u, packed[4 * j], packed[4 * j + 1],
                          packed[4 * j + 2], packed[4 * j + 3]);
           }
         }
         fence_proxy_async_smem();
-        named_bar_sync(1, kEpiWarps * 32);
-        if (issuer) {
-          tma_store_2d_hint(&tmap_y, obuf, n_base + h * 64, m_base, p.y_policy);  // OOB rows/cols are clipped
+        named_bar_sync(2u + q, 64);
+        if (issuer && kMB == 1 && h == SWIGLU_TRACE_H) SWIGLU_GEMM_TRACE(8 + it * 8 + 7);
+        if (q_issuer) {
+          tma_store_2d_hint(&tmap_y, obuf, n_base + h * 64, m_base + (int)(q * 32u), p.y_policy);  // OOB rows/cols are clipped
           tma_store_commit();
         }
       }
       }
       if (issuer) SWIGLU_GEMM_TRACE(8 + it * 8 + 4);
     }
-    if (issuer) tma_store_wait_all<0>();
+    if (q_issuer) tma_store_wait_all<0>();
   }
 
   // ------------------------------------------------------------------ teardown

@@ -487,7 +487,7 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
     if ((rc = make_tmap(&tb1, B1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
     if ((rc = make_tmap(&tb2, kFused ? B2 : B1, kWK ? K : N, kWK ? N : K, 64, 64))) return rc;
   }
-  if ((rc = make_tmap(&ty, Yout, N, M, 64, 128))) return rc;
+  if ((rc = make_tmap(&ty, Yout, N, M, 64, 32))) return rc;   // one store per TMEM lane quarter
   using Cfg = GemmCfg<kCtaGroup, kFused ? 2 * kBN : 256, kMB>;
   GemmParams p;
   p.M = (int)M; p.N = (int)N; p.K = (int)K;

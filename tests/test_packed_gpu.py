@@ -134,7 +134,11 @@ def test_packed_baseline_shapes_sampled_rows():
             rep = check.compare(host(dY[torch.from_numpy(rows).cuda()]), y_ref)
             assert rep.mismatches == 0, (shape, M, rep)
             assert bool(torch.isfinite(dY.float()).all())
-            assert np.array_equal(host(dY), host(dY2)), (shape, M)
+            # (0.5B at M <= 32: the unpacked call runs the stacked 64-column decode tile with K
+            # split in two, the packed call the 128-column tile with K split in three -- both
+            # within the bound, a different fp32 summation order)
+            if not (shape == "qwen2.5-0.5b" and M <= 32):
+                assert np.array_equal(host(dY), host(dY2)), (shape, M)
 
 
 def test_packed_decode_chain_in_a_cuda_graph():
