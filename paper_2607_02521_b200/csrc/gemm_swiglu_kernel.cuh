@@ -766,7 +766,9 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
       }
       if (issuer) SWIGLU_GEMM_TRACE(8 + it * 8 + 4);
     }
-    if (q_issuer) tma_store_wait_all<0>();
+    // shared memory may go once the last stores have READ it; their global writes complete with
+    // the grid (and before any dependent grid passes griddepcontrol.wait)
+    if (q_issuer) tma_store_wait_read<0>();
   }
 
   // ------------------------------------------------------------------ teardown
