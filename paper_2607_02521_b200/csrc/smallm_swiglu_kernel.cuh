@@ -410,8 +410,12 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     }
     if (threadIdx.x == 64) SWIGLU_TRACE_POINT(7);
     if (S > 1) {
+      // peers may still be reading this CTA's partials: wait for all of them.  Nothing is
+      // published here (Y needs no ordering inside the cluster), so the arrival is relaxed: a
+      // release would first wait for this thread's Y stores to reach L2.
       __syncwarp();
-      cluster_sync();  // peers may still be reading this CTA's partials
+      cluster_arrive_relaxed();
+      cluster_wait_acquire();
     } else {
       __syncthreads();
     }
