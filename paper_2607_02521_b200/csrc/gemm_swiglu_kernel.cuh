@@ -774,7 +774,9 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
   // ------------------------------------------------------------------ teardown
   __syncwarp();
   tcgen05_fence_before();
-  if (kCtaGroup == 2) cluster_sync(); else __syncthreads();
+  // (relaxed arrival: the barrier only says "this CTA no longer touches its peers' shared memory,
+  // barriers or TMEM"; there is nothing to publish, so no release that drains the stores first)
+  if (kCtaGroup == 2) { cluster_arrive_relaxed(); cluster_wait_acquire(); } else __syncthreads();
   if (warp == 1) {
     tcgen05_fence_after();
     tmem_dealloc<kCtaGroup>(tmem_base, kTmemCols);
