@@ -170,12 +170,12 @@ int select_fused(int64_t M, int64_t N, int64_t K) {
   if (M <= 32) return kFusedSmallM;
   if (M <= 64) return few_tiles ? kFused1CtaN64 : kFusedSmallM;
   if (M <= 128) return few_tiles ? kFused1CtaN64 : kFused1Cta;
-  // M > 128: a CTA-pair kernel.  The 512-row super tile moves a quarter less data per FLOP and
-  // these calls are power-bound (profiles/r02_variant_sweep_super_tile.md: +1-6 % in short
-  // bursts, +3-5 % under sustained load) -- where each tile's mainloop is long enough to
-  // amortise the skewed tile boundary (K >= 2048: the 1.5B-class shapes are 5 % slower with it)
-  // and the 512-row granularity does not cost more in wave quantisation than it gains.
-  if (M > 512 && K >= 2048 && wave_eff_super(M, N, 74) >= wave_eff_pair(M, N, K, 74) - 0.03)
+  // M > 128: a CTA-pair kernel.  The 512-row super tile moves a quarter less data per FLOP: these
+  // calls are power-bound under load and L2->SM-bound at high clocks (
+  // profiles/r02b_variant_sweep_super_tile.md: +1-9 % in short bursts, +3-7 % sustained, at
+  // every K from 896 up once the accumulator hand-back stopped costing 1.2 us per region) --
+  // wherever the 512-row granularity does not cost more in wave quantisation than it gains.
+  if (M > 512 && K >= 768 && wave_eff_super(M, N, 74) >= wave_eff_pair(M, N, K, 74) - 0.03)
     return kFused2CtaMB2;
   return kFused2Cta;
 }
@@ -187,7 +187,7 @@ int select_unfused(int64_t M, int64_t N, int64_t K) {
   // Gate and Up -- so that fused vs unfused compares fusion, not tile shapes.
   if (M <= 128) return kUnfusedSmallM;
   // Large M: the same super-tile rule as the fused path (same mainloop, same power argument).
-  if (M > 512 && K >= 2048) {
+  if (M > 512 && K >= 768) {
     const int64_t tiles = ((M + 255) / 256) * ((N + 255) / 256), rem = tiles % 74;
     const double eff_pair = (double)tiles / 74 / (double)(tiles / 74 + (rem ? 1 : 0));
     if (wave_eff_super(M, N, 74, 256) >= eff_pair - 0.03) return kUnfused2CtaMB2;

@@ -47,7 +47,7 @@ def test_version_status_strings_and_variant_table(lib):
 
 
 def test_large_m_dispatch_table(lib):
-    """Host-only table (no CUDA call): the 512-row super tile for M > 512 with K >= 2048 where its
+    """Host-only table (no CUDA call): the 512-row super tile for M > 512 with K >= 768 where its
     wave efficiency is within 3 points of the 256-row pair kernel's, the pair kernel otherwise
     (profiles/r02b_variant_sweep_super_tile.md); same rule for the unfused GEMM."""
     name = lambda M, N, K, unfused=False: B.swiglu_variant_name(
@@ -58,10 +58,12 @@ def test_large_m_dispatch_table(lib):
             assert "512x256" in name(M, N, K, unfused=True), (M, N, K)
         for M in (129, 256, 512):
             assert name(M, N, K) == "fused_2cta_256x128", (M, N, K)
-    for K, N in ((896, 4864), (1536, 8960)):            # short K: the skewed tile boundary does not amortise
-        for M in (256, 1024, 4096, 8192):
+    for K, N in ((896, 4864), (1536, 8960)):            # short K too, from M = 1024 up
+        for M in (1024, 4096, 8192):
+            assert "512x128" in name(M, N, K), (M, N, K)
+        for M in (256, 512, 768):
             assert name(M, N, K) == "fused_2cta_256x128", (M, N, K)
-            assert "256x256" in name(M, N, K, unfused=True), (M, N, K)
+    assert name(4096, 4864, 512) == "fused_2cta_256x128"   # fewer than 12 k-blocks per tile
     # no workspace for the super tile (its last wave is cut into row-block / quarter units, not in K)
     assert B.swiglu_workspace_bytes(8192, 29568, 8192, unfused=False) == 0
     assert B.swiglu_workspace_bytes(512, 29568, 8192, unfused=False) > 0     # pair kernel, K-split tail
