@@ -702,6 +702,17 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   const int64_t grid = n_tiles * p.ksplit;
   int64_t pf = (32ll << 20) / (grid * 2 * Cfg::kWBytes);
   if (pf > kSmallPrefetchMax) pf = kSmallPrefetchMax;
+  // ... and no more than 4 k-blocks or a third of the CTA's K-range: the prefetch only has to
+  // cover the start-up latency behind griddepcontrol.wait; anything more competes with the
+  // PREVIOUS call's weight stream for HBM (1.5B M=16, cap 0 / 2 / 4 / 8 / 14 k-blocks: 10.66 /
+  // 10.44 / 10.42 / 10.46 / 11.51 us; 0.5B: 6.10 / 5.61 / 5.79 / 6.11 / 6.10; 7B: 40.8 / 40.0 / 39.5 /
+  // 39.7 / 39.7 -- profiles/r02b_decode_stack_sweep.md)
+  {
+    const int64_t kb_per_cta = (k_blocks + p.ksplit - 1) / p.ksplit;
+    int64_t cap = kb_per_cta / 3 < 4 ? kb_per_cta / 3 : 4;
+    if (cap < 1) cap = 1;
+    if (pf > cap) pf = cap;
+  }
   if (env().no_prefetch) pf = 0;
   p.prefetch_blocks = (int)pf;
 #ifdef SWIGLU_TRACE
