@@ -69,6 +69,7 @@ struct GemmParams {
   float* split_ws;  // [tail tile][CTA of the group][s][256 columns / 4][128 rows] float4 partials
   int* split_ctr;   // [tail tile][CTA of the group] arrival counters, zero between launches
   int early_issue;      // 1: fill the ring before the CTA-wide setup barrier (small grids)
+  int early_prefetch;   // ... after an L2 prefetch of this many weight k-blocks ahead of griddepcontrol.wait
   unsigned long long w_policy, a_policy;  // L2 eviction-priority hints of the weight / A loads
   unsigned long long y_policy;            // ... and of the Y stores
   unsigned long long* clk;  // optional {SM cycles, globaltimer ns} of CTA 0 (swiglu_set_clock_probe)
@@ -439,9 +440,21 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
         // The producer needs only the barriers it has just initialised: fill the ring before
         // the CTA-wide setup barrier so TMEM allocation overlaps the first loads' latency.
         if (p.early_issue && group_id < total_tiles) {  // (host: never with a K-split tail)
-          pdl_wait_prior_grid();
           int tm, n_base, w;
           decode_tile_w<kOutCols>(p, group_id, tm, n_base, w);
+          if constexpr (kWMode == kWeightsKN) {
+            // L2 prefetch (a hint) of the first few weight k-blocks ahead of the grid dependency,
+            // as in the decode kernel: covers the start-up latency behind griddepcontrol.wait
+            for (int kb = 0; kb < p.early_prefetch && kb < k_blocks; ++kb) {
+              tma_prefetch_l2_2d(&tmap_b1, n_base, kb * BK);
+              tma_prefetch_l2_2d(&tmap_b2, n_base, kb * BK);
+              if (w == 128) {
+                tma_prefetch_l2_2d(&tmap_b1, n_base + 64, kb * BK);
+                tma_prefetch_l2_2d(&tmap_b2, n_base + 64, kb * BK);
+              }
+            }
+          }
+          pdl_wait_prior_grid();
           for (; pre < kStages && pre < k_blocks; ++pre)
             issue_loads(pre, pre, tm * BM, n_base, w);  // fresh ring: nothing to wait for
         }

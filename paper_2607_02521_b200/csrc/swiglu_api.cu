@@ -555,6 +555,12 @@ int launch_gemm(const DeviceState& d, const void* A, const void* B1, const void*
   // one tile per CTA (a short, HBM-bound call): fill the TMA ring before the setup barrier
   p.early_issue = (kCtaGroup == 1 && kFused && tiles <= groups && tail.ksplit == 0 && !env().no_early);
   {
+    const int64_t kb = (K + kBKe - 1) / kBKe;
+    // (same cap as the decode kernel; M = 128, 0 / 2 / 4 / 8 k-blocks: 1.5B 11.29 / 11.08 / 11.13 /
+    // 11.61 us, 7B 41.96 / 41.37 / 40.90 / 40.15 us)
+    p.early_prefetch = env().no_prefetch ? 0 : (int)(kb / 3 < 4 ? kb / 3 : 4);
+  }
+  {
     const uint64_t pol[3] = {sm100::kEvictNormal, sm100::kEvictFirst, sm100::kEvictLast};
     p.w_policy = (p.m_tiles == 1 && !env().no_w_evict_first) ? sm100::kEvictFirst : sm100::kEvictNormal;
     p.a_policy = sm100::kEvictNormal;
