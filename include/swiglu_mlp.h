@@ -102,6 +102,26 @@ int swiglu_mlp_unfused_ex(const void* A, const void* W1, const void* W2, void* Y
                           int variant, void* stream);
 
 /*
+ * No-allocation form of the unfused path, for callers that cannot allocate device memory (code
+ * under CUDA-graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same
+ * arguments, result and kernels as swiglu_mlp_unfused, but the bf16 Gate / Up scratch
+ * (2 * round_up(M*N*2, 256) bytes) lives in ONE file-scope `static __device__` array of
+ * SWIGLU_STATIC_SCRATCH_BYTES (32 MiB) inside the library: every GPU that loads the library holds
+ * those 32 MiB until the process exits.  The call makes no cudaMalloc / cudaMallocAsync / cudaFree
+ * and no allocating library call; its only set-up is one cudaGetSymbolAddress per device.
+ *   - Sizes whose scratch exceeds the array (M*N > ~8.39 M elements, e.g. more than 283 rows at
+ *     N = 29568) are rejected with SWIGLU_ERR_WORKSPACE before any CUDA call; use
+ *     swiglu_mlp_unfused_ex with a caller workspace for those.
+ *   - Every call on a device shares the array, which keeps the previous call's contents.  Nothing
+ *     in it has to start at zero: the GEMMs write every Gate / Up element of [0,M) x [0,N) before
+ *     the elementwise kernel reads it.  Calls that OVERLAP on the GPU (two streams, two host
+ *     threads, a graph replayed next to an eager call) race on it: the caller must serialise them.
+ */
+#define SWIGLU_STATIC_SCRATCH_BYTES (32u << 20)
+int swiglu_mlp_unfused_static(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                              int64_t N, int64_t K, void* stream);
+
+/*
  * Other gated activations of the GLU family ("gated linear unit variants
  * (GEGLU, SwiGLU, ReGLU)"; line 392 future-work item 4): Y = bf16(act(A.W1) * (A.W2)) with the
  * same tensors, layout, numeric contract (fp32 activation on the fp32 accumulators, one RNE

@@ -34,7 +34,7 @@ EXPORTS = (
     "swiglu_release", "swiglu_release_stream", "swiglu_reload_env", "swiglu_tensor_map_cache_stats",
     "swiglu_set_clock_probe", "swiglu_packed_weight_bytes", "swiglu_pack_weights",
     "swiglu_mlp_packed", "swiglu_glu_mlp_packed", "swiglu_launch_floor_probe",
-    "swiglu_mlp_fp8", "swiglu_mlp_fp8_ex",
+    "swiglu_mlp_fp8", "swiglu_mlp_fp8_ex", "swiglu_mlp_unfused_static",
 )
 
 
@@ -58,7 +58,7 @@ def load():
             "(or __graft_entry__.build()); there is no CPU or PyTorch fallback")
     lib = ctypes.CDLL(LIB_PATH)
     p, i64, sz, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_size_t, ctypes.c_int
-    for name in ("swiglu_mlp", "swiglu_mlp_unfused"):
+    for name in ("swiglu_mlp", "swiglu_mlp_unfused", "swiglu_mlp_unfused_static"):
         f = getattr(lib, name)
         f.argtypes, f.restype = [p, p, p, p, i64, i64, i64, p], ci
     for name in ("swiglu_mlp_ex", "swiglu_mlp_unfused_ex"):
@@ -169,6 +169,17 @@ def swiglu_mlp_unfused(A, W1, W2, Y, M=None, N=None, K=None, stream=None) -> Non
     m, n, k = _dims(A, W1, W2, Y, M, N, K)
     _check(load().swiglu_mlp_unfused(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), m, n, k,
                                      _stream(stream)))
+
+
+STATIC_SCRATCH_BYTES = 32 << 20   # SWIGLU_STATIC_SCRATCH_BYTES
+
+
+def swiglu_mlp_unfused_static(A, W1, W2, Y, M=None, N=None, K=None, stream=None) -> None:
+    """swiglu_mlp_unfused with its Gate/Up scratch in the library's static device array: no
+    allocation; sizes beyond STATIC_SCRATCH_BYTES are rejected; overlapping calls race."""
+    m, n, k = _dims(A, W1, W2, Y, M, N, K)
+    _check(load().swiglu_mlp_unfused_static(_ptr(A), _ptr(W1), _ptr(W2), _ptr(Y), m, n, k,
+                                            _stream(stream)))
 
 
 def swiglu_mlp_ex(A, W1, W2, Y, M=None, N=None, K=None, workspace=None, workspace_bytes=0,

@@ -16,6 +16,11 @@
 #include "gemm_swiglu_kernel.cuh"
 #include "smallm_swiglu_kernel.cuh"
 
+// Scratch of swiglu_mlp_unfused_static (include/swiglu_mlp.h): bf16 Gate | Up of one call.  In HOST
+// code this name is only a stand-in for the symbol, not a device address: the address is taken
+// once per device with cudaGetSymbolAddress (static_scratch_address below) and passed to the kernels.
+static __device__ __align__(256) unsigned char g_static_scratch[SWIGLU_STATIC_SCRATCH_BYTES];
+
 namespace {
 
 using swiglu::kWeightsKN;
@@ -1001,6 +1006,25 @@ int run_unfused(const void* A, const void* W1, const void* W2, void* Y, int64_t 
   return launch_silu_mul(*d, G, U, Y, M * N, act, stream);
 }
 
+// Device address of g_static_scratch on the CURRENT device, resolved once per device.
+std::mutex g_static_mu;
+void* g_static_addr[64] = {nullptr};
+int static_scratch_address(void** out) {
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return fail(SWIGLU_ERR_CUDA, "device index %d out of range", dev);
+  std::lock_guard<std::mutex> lk(g_static_mu);
+  if (!g_static_addr[dev]) {
+    void* ptr = nullptr;
+    CUDA_TRY(cudaGetSymbolAddress((void**)&ptr, g_static_scratch));  // `dev` is current
+    if (!ptr || ((uintptr_t)ptr & 255u))
+      return fail(SWIGLU_ERR_CUDA, "static scratch resolved to a bad address %p", ptr);
+    g_static_addr[dev] = ptr;
+  }
+  *out = g_static_addr[dev];
+  return SWIGLU_OK;
+}
+
 }  // namespace
 
 // ====================================================================== C ABI
@@ -1034,6 +1058,23 @@ int swiglu_mlp_unfused_ex(const void* A, const void* W1, const void* W2, void* Y
                           int64_t N, int64_t K, void* workspace, size_t workspace_bytes,
                           int variant, void* stream) {
   return run_unfused(A, W1, W2, Y, M, N, K, workspace, workspace_bytes, false, variant,
+                     swiglu::kActSilu, 0, (cudaStream_t)stream);
+}
+
+int swiglu_mlp_unfused_static(const void* A, const void* W1, const void* W2, void* Y, int64_t M,
+                              int64_t N, int64_t K, void* stream) {
+  int rc = validate(A, W1, W2, Y, M, N, K);  // no CUDA call yet
+  if (rc) return rc;
+  if (M == 0) return SWIGLU_OK;
+  const size_t need = workspace_for(M, N, K, 1, -1);
+  if (need > (size_t)SWIGLU_STATIC_SCRATCH_BYTES)
+    return fail(SWIGLU_ERR_WORKSPACE,
+                "M=%lld x N=%lld needs %zu bytes of Gate/Up scratch; the static scratch of "
+                "swiglu_mlp_unfused_static holds %u (use swiglu_mlp_unfused_ex with a caller workspace)",
+                (long long)M, (long long)N, need, (unsigned)SWIGLU_STATIC_SCRATCH_BYTES);
+  void* scratch = nullptr;
+  if ((rc = static_scratch_address(&scratch))) return rc;
+  return run_unfused(A, W1, W2, Y, M, N, K, scratch, SWIGLU_STATIC_SCRATCH_BYTES, false, -1,
                      swiglu::kActSilu, 0, (cudaStream_t)stream);
 }
 
