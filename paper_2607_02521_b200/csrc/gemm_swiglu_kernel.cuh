@@ -627,6 +627,9 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     for (int t = group_id; t < total_tiles; t += num_groups, ++it) {
       const TileUnit tu = decode_unit<kOutCols, kMB>(p, t, k_blocks);
       const int n_base = tu.n_base, w = tu.w;
+      // does the MMA thread wait for this tile's accumulator region(s) again?  (kMB = 1: stage
+      // it & 1 is reused two tiles later; kMB = 2: by the next tile)
+      const bool hand_back = t + (kMB == 2 ? 1 : 2) * num_groups < total_tiles;
       const int chunks = kFused ? w / 64 : kChunks;  // 64-column chunks in this tile
 #pragma unroll 1
       for (int mb = 0; mb < tu.nmb; ++mb) {  // accumulator regions of the tile (kMB = 2: row blocks)
@@ -661,7 +664,7 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
           }
           tcgen05_fence_before();
           __syncwarp();
-          if (lane == 0) {  // TMEM stage drained (relaxed: see the hand-back in the chunk loop)
+          if (lane == 0 && hand_back) {  // TMEM stage drained (relaxed: see the hand-back in the chunk loop)
             if constexpr (kCtaGroup == 2) mbar_arrive_relaxed_cluster(leader_acc_empty0 + 8u * as);
             else mbar_arrive_relaxed(acc_empty_bar(as));
           }
@@ -750,12 +753,14 @@ gemm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
             // last TMEM read of this tile is done: hand the accumulator stage back to the MMA
             tcgen05_fence_before();
             __syncwarp();
-            if (lane == 0) {
+            if (lane == 0 && hand_back) {
               // RELAXED arrive: the only thing the MMA thread needs from this warp is that its
               // TMEM reads are over, and tcgen05.wait::ld above has already retired them into
               // registers; there is no memory to publish.  (A release at cluster scope here cost
               // 1.2 us per hand-back -- it drains this thread's earlier stores first: measured
-              // 3.4 -> 2.2 us per 128x128 tile epilogue.)
+              // 3.4 -> 2.2 us per 128x128 tile epilogue.)  Not sent at all when the
+              // MMA thread will not reuse the region (hand_back): no remote arrival may still be
+              // in flight towards the pair leader's shared memory when that CTA exits.
               if constexpr (kCtaGroup == 2) mbar_arrive_relaxed_cluster(leader_acc_empty0 + 8u * as);
               else mbar_arrive_relaxed(acc_empty_bar(as));
             }

@@ -335,7 +335,7 @@ int get_device_state(DeviceState** out) {
 
 // Tensor-map cache (a0: "build or fetch cached CUtensorMaps").  A map is a pure function of
 // (base, dims, box): a cached copy can never be stale, whatever happened to the
-// allocation in between.  Thread-local and direct-mapped, so the hot path takes no lock.
+// allocation in between.  Thread-local (the hot path takes no lock), 64 sets x 4 ways, LRU.
 struct TmapKey {
   const void* base; int64_t d0, d1, d2; uint32_t b0, b1, b2; uint32_t esize;  // 2 = bf16, 1 = fp8
   int64_t pitch1;  // rows between consecutive d2 slices (>= d1; 0 = dense)
@@ -344,9 +344,11 @@ struct TmapKey {
            b2 == o.b2 && esize == o.esize && pitch1 == o.pitch1;
   }
 };
-struct TmapSlot { bool used = false; TmapKey key; CUtensorMap map; };
+struct TmapSlot { bool used = false; uint64_t tick = 0; TmapKey key; CUtensorMap map; };
 constexpr int kTmapSlots = 256;
+constexpr int kTmapWays = 4;
 thread_local TmapSlot t_tmaps[kTmapSlots];
+thread_local uint64_t t_tmap_tick = 0;
 thread_local uint64_t t_tmap_hits = 0, t_tmap_misses = 0;
 
 // bf16 (or 1-byte) tensor, dense row-major, dims innermost first (d2 == 0: 2-D), box b0 x b1
@@ -375,18 +377,32 @@ int cached_tmap(CUtensorMap* out, const TmapKey& key) {
   h ^= ((uint64_t)key.d0 * 0xC2B2AE3D27D4EB4Full) ^ ((uint64_t)key.d1 * 0x165667B19E3779F9ull) ^
        ((uint64_t)key.d2 * 0x27D4EB2F165667C5ull) ^ ((uint64_t)key.b1 << 7) ^ ((uint64_t)key.b2 << 17) ^
        ((uint64_t)key.esize << 27) ^ ((uint64_t)key.pitch1 << 31);
-  TmapSlot& slot = t_tmaps[(h >> 40) & (kTmapSlots - 1)];
-  if (slot.used && slot.key == key) {
-    ++t_tmap_hits;
-    *out = slot.map;
-    return SWIGLU_OK;
+  // four-way set associative with least-recently-used replacement (t_tmap_tick stamps every use):
+  // the handful of live maps of one call -- A, W1, W2, Y -- cannot evict each other on every call
+  // when their hashes collide, as they would in a direct-mapped table
+  const uint32_t set = (uint32_t)(h >> 40) & (kTmapSlots / kTmapWays - 1);
+  TmapSlot* ways = t_tmaps + (size_t)set * kTmapWays;
+  ++t_tmap_tick;
+  for (int w = 0; w < kTmapWays; ++w) {
+    if (ways[w].used && ways[w].key == key) {
+      ++t_tmap_hits;
+      ways[w].tick = t_tmap_tick;
+      *out = ways[w].map;
+      return SWIGLU_OK;
+    }
   }
   ++t_tmap_misses;
   const int rc = encode_tmap(out, key);
   if (rc) return rc;
-  slot.used = true;
-  slot.key = key;
-  slot.map = *out;
+  int victim = 0;
+  for (int w = 0; w < kTmapWays; ++w) {
+    if (!ways[w].used) { victim = w; break; }
+    if (ways[w].tick < ways[victim].tick) victim = w;
+  }
+  ways[victim].used = true;
+  ways[victim].key = key;
+  ways[victim].map = *out;
+  ways[victim].tick = t_tmap_tick;
   return SWIGLU_OK;
 }
 
