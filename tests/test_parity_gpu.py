@@ -640,6 +640,33 @@ def test_invariants_on_gpu():
     assert np.all(np.abs(ys - yl) <= ATOL + RTOL * np.abs(yl))
 
 
+def test_chained_calls_of_mixed_shapes_stay_bit_identical():
+    """Back-to-back calls of different kernels on one stream (programmatic dependent launch: each
+    kernel's prologue overlaps its predecessor's tail; CTAs exit while cluster peers and the next
+    grid start): 1800 chained calls over the decode, 1-CTA, pair and super-tile kernels must
+    reproduce, bit for bit, the output each shape gave when it ran alone -- a stray barrier arrival
+    or an early shared-memory reuse would show up here as a trap, a hang or a differing output."""
+    shapes = [(256, 4864, 896), (300, 1160, 328), (16, 4864, 896), (1024, 4864, 896),
+              (700, 8960, 1536), (128, 8960, 1536), (2560, 1032, 200), (1, 8960, 1536), (513, 392, 1096)]
+    cases = []
+    for i, (M, N, K) in enumerate(shapes):
+        A, W1, W2 = inputs.make_case(M, N, K, seed=700 + i, std=0.05)
+        dA, dW1, dW2 = dev(A), dev(W1), dev(W2)
+        y0 = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
+        B.swiglu_mlp(dA, dW1, dW2, y0)
+        torch.cuda.synchronize()
+        cases.append((dA, dW1, dW2, y0, torch.empty_like(y0)))
+    A, W1, W2 = inputs.make_case(*shapes[1], seed=701, std=0.05)
+    assert_parity(host(cases[1][3]), oracle.swiglu_oracle(A, W1, W2)[0], "reference output")
+    for rnd in range(8):
+        for c in np.random.RandomState(rnd).permutation(len(cases) * 25) % len(cases):
+            dA, dW1, dW2, _, y = cases[c]
+            B.swiglu_mlp(dA, dW1, dW2, y)
+        torch.cuda.synchronize()
+        for (M, N, K), (_, _, _, y0, y) in zip(shapes, cases):
+            assert torch.equal(y.view(torch.int16), y0.view(torch.int16)), (rnd, M, N, K)
+
+
 def test_run_to_run_determinism():
     for M, N, K in [(16, 4864, 896), (300, 4864, 896)]:
         A, W1, W2 = inputs.make_case(M, N, K, seed=41)
