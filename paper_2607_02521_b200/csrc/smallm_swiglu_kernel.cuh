@@ -65,6 +65,7 @@ struct SmallParams {
   int M, N, K;
   int ksplit;         // cluster size S
   int prefetch_blocks;  // leading k-blocks of each CTA's weight stream to prefetch into L2
+  int packed_pre;       // kWeightsPacked: ring stages whose weight loads go out before griddepcontrol.wait
   int probe;          // launch-floor probe (swiglu_launch_floor_probe): 1 = prologue and teardown
                       // only (no loads, MMAs, reduction or stores); 0 = the real kernel
   long long ldy;      // = N
@@ -173,20 +174,27 @@ smallm_swiglu_kernel(const __grid_constant__ CUtensorMap tmap_a,
     if constexpr (kPacked) {
       // Packed weights are constants (header contract): their loads need not wait for the
       // previous kernel.  Fill the ring's weight half now; the A half follows the dependency.
+      const int pre = min(kStages, p.packed_pre);  // ring stages whose weights go out before the wait
       if (lane == 0 && live) {
-        for (int i = 0; i < kStages && kb_begin + i < kb_end; ++i) {
+        for (int i = 0; i < pre && kb_begin + i < kb_end; ++i) {
           mbar_arrive_expect_tx(full_bar(i), Cfg::kStageBytes);
           issue_w(kb_begin + i, i);
         }
       }
-      // the rest of the CTA's weight stream: L2 prefetch, one k-block per lane
-      const int kb = kb_begin + kStages + (int)lane;
+      // the next blocks of the CTA's weight stream: L2 prefetch, one k-block per lane
+      const int kb = kb_begin + pre + (int)lane;
       if (live && (int)lane < p.prefetch_blocks && kb < kb_end)
         tma_prefetch_l2_3d(&tmap_w1, 0, kb * kBKe, n_tile * (kTileN / 32));
       if (lane == 0 && live) {
         pdl_wait_prior_grid();  // A may be the previous kernel's output
         SWIGLU_TRACE_POINT(2);
-        for (int i = 0; i < kStages && kb_begin + i < kb_end; ++i) issue_a(kb_begin + i, i);
+        for (int i = 0; i < kStages && kb_begin + i < kb_end; ++i) {
+          if (i >= pre) {
+            mbar_arrive_expect_tx(full_bar(i), Cfg::kStageBytes);
+            issue_w(kb_begin + i, i);
+          }
+          issue_a(kb_begin + i, i);
+        }
       }
     } else {
       // L2 prefetch of this CTA's weight stream (hint; legal before griddepcontrol.wait)

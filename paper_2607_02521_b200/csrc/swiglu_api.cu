@@ -742,6 +742,10 @@ int launch_smallm_mp(const DeviceState& d, const void* A, const void* W1, const 
   }
   if (env().no_prefetch) pf = 0;
   p.prefetch_blocks = (int)pf;
+  // prepacked weights: two ring stages of real weight loads go out ahead of the grid dependency
+  // (all of the ring / 4 / 2 / 1 / 0 stages, M = 16: 0.5B 6.25 / - / 5.97 / 6.06 / 6.39 us, 1.5B
+  // 10.18 / - / 9.95 / 10.40 / 11.12 us: like the L2 prefetch, more only fights the previous call)
+  p.packed_pre = 2;
 #ifdef SWIGLU_TRACE
   p.trace = g_trace;
 #endif
