@@ -157,6 +157,16 @@ double wave_eff_super(int64_t M, int64_t N, int pairs, int cols = 128) {
   return work / pairs / waves;
 }
 
+// Three or five 128-row tiles (256 < M <= 384, 512 < M <= 640): the pair kernels pad M to a
+// multiple of 256 and would compute a quarter / a sixth more rows than the 1-CTA kernel, which
+// outweighs its heavier L2 traffic (profiles/r02b_variant_sweep_odd_m.md: M = 384 / 640 -- 0.5B
+// 13.8 -> 9.9 / 15.3 -> 14.4 us, 7B 106 -> 90 / 162 -> 145, 72B 380 -> 325 / 580 -> 497; ties at 1.5B;
+// from seven row tiles on the two are within noise or the pair kernels win).
+bool odd_row_tiles(int64_t M) {
+  const int64_t r = (M + 127) / 128;
+  return r == 3 || r == 5;
+}
+
 // Measured dispatch (table regenerated from bench sweeps).
 int select_fused(int64_t M, int64_t N, int64_t K) {
   const int forced = env().variant;
@@ -180,6 +190,7 @@ int select_fused(int64_t M, int64_t N, int64_t K) {
   // profiles/r02b_variant_sweep_super_tile.md: +1-9 % in short bursts, +3-7 % sustained, at
   // every K from 896 up once the accumulator hand-back stopped costing 1.2 us per region) --
   // wherever the 512-row granularity does not cost more in wave quantisation than it gains.
+  if (odd_row_tiles(M)) return kFused1Cta;
   if (M > 512 && K >= 768 && wave_eff_super(M, N, 74) >= wave_eff_pair(M, N, K, 74) - 0.03)
     return kFused2CtaMB2;
   return kFused2Cta;

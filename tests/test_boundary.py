@@ -56,8 +56,10 @@ def test_large_m_dispatch_table(lib):
         for M in (1024, 2048, 4096, 8192):
             assert "512x128" in name(M, N, K), (M, N, K)
             assert "512x256" in name(M, N, K, unfused=True), (M, N, K)
-        for M in (129, 256, 512):
+        for M in (129, 256, 512, 768):
             assert name(M, N, K) == "fused_2cta_256x128", (M, N, K)
+        for M in (300, 384, 600, 640):     # three / five 128-row tiles: no padded half tile row
+            assert name(M, N, K) == "fused_1cta_128x128", (M, N, K)
     for K, N in ((896, 4864), (1536, 8960)):            # short K too, from M = 1024 up
         for M in (1024, 4096, 8192):
             assert "512x128" in name(M, N, K), (M, N, K)
