@@ -640,6 +640,26 @@ def test_invariants_on_gpu():
     assert np.all(np.abs(ys - yl) <= ATOL + RTOL * np.abs(yl))
 
 
+def test_random_shapes_through_the_automatic_dispatch():
+    """Seeded random (M, N, K) -- decode sizes, the ridge, several waves; any multiple of 8 for N and
+    K -- through `swiglu_mlp` and `swiglu_mlp_unfused` with automatic dispatch, every output against
+    the oracle: whatever variant, tail plan and split the tables pick.  (A 2000-shape run of the same
+    generator was clean when the dispatch rules of round 2 went in.)"""
+    rs = np.random.RandomState(20260711)
+    done = 0
+    while done < 60:
+        M = int(rs.choice([rs.randint(1, 130), rs.randint(129, 1100), rs.randint(1000, 3500)]))
+        N = 8 * int(rs.randint(1, 900))
+        K = 8 * int(rs.choice([rs.randint(1, 40), rs.randint(40, 300)]))
+        if M * N * K > 3e9:
+            continue
+        done += 1
+        A, W1, W2 = inputs.make_case(M, N, K, seed=int(rs.randint(1 << 30)), std=0.05)
+        y_ref, _ = oracle.swiglu_oracle(A, W1, W2)
+        assert_parity(run("auto", -1, A, W1, W2), y_ref, ("auto", M, N, K))
+        assert_parity(run("auto_unfused", -1, A, W1, W2), y_ref, ("auto_unfused", M, N, K))
+
+
 def test_chained_calls_of_mixed_shapes_stay_bit_identical():
     """Back-to-back calls of different kernels on one stream (programmatic dependent launch: each
     kernel's prologue overlaps its predecessor's tail; CTAs exit while cluster peers and the next
