@@ -31,8 +31,11 @@
  * with stream-ordered allocation (cudaMallocAsync / cudaFreeAsync on `stream`), so growth never
  * synchronises and never frees memory that earlier work on that stream still uses.  A stream
  * that is being captured is refused (SWIGLU_ERR_WORKSPACE): use the _ex forms with a caller
- * workspace under CUDA-graph capture.  swiglu_release_stream / swiglu_release give the buffers
- * back.  The fused entry points need no workspace and are always capturable.
+ * workspace under CUDA-graph capture, or swiglu_mlp_unfused_static (scratch in a static device
+ * array of the library: no allocation at all, bounded size).  swiglu_release_stream /
+ * swiglu_release give the buffers back.  The fused entry points need no workspace and are always
+ * capturable (the optional K split of their last wave uses a fixed-size per-stream buffer when
+ * one may be created, or the caller's through swiglu_mlp_ex; under capture it is skipped).
  *
  * Errors: a swiglu_status return code; the library never throws, aborts or prints, and the
  * device-pointer compute entry points never synchronise (the host-buffer forms and
